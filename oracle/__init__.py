@@ -1,0 +1,134 @@
+"""ORACLE — test infrastructure, not the product.
+
+ctypes wrapper around oracle/rtvd_oracle.cpp (plain CPU relaxing-TVD update written from PAPER.md §2.2/§3.1).
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may import this.
+It imports nothing from the CUDA package and the CUDA package imports nothing from here.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+NCOMP, PS, NGHOST, NP = 5, 16, 3, 22
+IN_GROUP = NCOMP * NP ** 3      # 53 240 values per padded group
+OUT_GROUP = NCOMP * PS ** 3     # 20 480 values per interior
+FACE_GROUP = 3 * 3 * NCOMP * PS * PS
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        for sfx, ct in (("f32", ctypes.c_float), ("f64", ctypes.c_double)):
+            p = ctypes.c_void_p
+            getattr(L, "oracle_van_leer_" + sfx).restype = ct
+            getattr(L, "oracle_van_leer_" + sfx).argtypes = [ct, ct]
+            getattr(L, "oracle_cell_fluxes_" + sfx).restype = None
+            getattr(L, "oracle_cell_fluxes_" + sfx).argtypes = [p, ct, ctypes.c_int, p, p, p]
+            getattr(L, "oracle_row_update_" + sfx).restype = None
+            getattr(L, "oracle_row_update_" + sfx).argtypes = [p, p, ctypes.c_int, ct, ct, ctypes.c_int, ctypes.c_int, p, p]
+            getattr(L, "oracle_hydro_advance_" + sfx).restype = ctypes.c_longlong
+            getattr(L, "oracle_hydro_advance_" + sfx).argtypes = [p, p, ctypes.c_longlong, ctypes.c_int, ct, ct, ct,
+                                                                 ctypes.c_int, ctypes.c_int, p, p, ctypes.c_int]
+        L.oracle_count_ops.restype = None
+        L.oracle_count_ops.argtypes = [ctypes.c_void_p]
+        L.oracle_has_openmp.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _sfx(dtype):
+    dtype = np.dtype(dtype)
+    if dtype == np.float32:
+        return "f32"
+    if dtype == np.float64:
+        return "f64"
+    raise TypeError("oracle computes in float32 or float64, got %s" % dtype)
+
+
+def van_leer(a, b, dtype=np.float64):
+    """Eq.11 on two scalars."""
+    return getattr(lib(), "oracle_van_leer_" + _sfx(dtype))(float(a), float(b))
+
+
+def cell_fluxes(u, gamma, dtype=np.float64, c_mode=0):
+    """Cell-centred (F^R, F^L, c) of one cell, u = (rho, m_n, m_t1, m_t2, e) (Eq.8)."""
+    dt = np.dtype(dtype)
+    u = np.ascontiguousarray(u, dtype=dt)
+    assert u.shape == (NCOMP,)
+    FR, FL, c = np.empty(NCOMP, dt), np.empty(NCOMP, dt), np.empty(1, dt)
+    getattr(lib(), "oracle_cell_fluxes_" + _sfx(dt))(u.ctypes.data, dt.type(gamma), c_mode, FR.ctypes.data,
+                                                    FL.ctypes.data, c.ctypes.data)
+    return FR, FL, c[0]
+
+
+def row_update(u, k, gamma, dtype=None, c_mode=0, limiter_on=1, want_half=False, want_flux=False):
+    """One 1-D relaxing-TVD update of a row.
+
+    u: [5][N] row-local components (rho, m_n, m_t1, m_t2, e).  Returns unew [5][N] (cells 3..N-4 updated, the rest
+    copied), plus optionally the midpoint state u^{t+dt/2} and the time-centred interface fluxes F_{n+1/2}.
+    """
+    dt = np.dtype(dtype if dtype is not None else u.dtype)
+    u = np.ascontiguousarray(u, dtype=dt)
+    assert u.ndim == 2 and u.shape[0] == NCOMP and u.shape[1] >= 7
+    N = u.shape[1]
+    unew = np.empty_like(u)
+    uh = np.empty_like(u) if want_half else None
+    fh = np.empty_like(u) if want_flux else None
+    getattr(lib(), "oracle_row_update_" + _sfx(dt))(u.ctypes.data, unew.ctypes.data, N, dt.type(k), dt.type(gamma),
+                                                   c_mode, limiter_on,
+                                                   uh.ctypes.data if want_half else None,
+                                                   fh.ctypes.data if want_flux else None)
+    res = (unew,)
+    if want_half:
+        res += (uh,)
+    if want_flux:
+        res += (fh,)
+    return res if len(res) > 1 else unew
+
+
+def hydro_advance(inp, dt, dh, gamma, backward=0, dtype=None, ghost=NGHOST, c_mode=0, want_face_flux=False,
+                  want_maxspeed=False, n_threads=1, return_bad=False):
+    """One 3-sweep pass over a batch of patch groups.
+
+    inp: [G][5][22][22][22].  Returns out [G][5][16][16][16] (+ face flux [G][3][3][5][16][16], + maxspeed [G]).
+    Raises if any cell met on the way has rho <= 0 or P <= 0 unless return_bad=True (reading R7).
+    """
+    dtp = np.dtype(dtype if dtype is not None else inp.dtype)
+    a = np.ascontiguousarray(inp, dtype=dtp)
+    assert a.ndim == 5 and a.shape[1:] == (NCOMP, NP, NP, NP), a.shape
+    G = a.shape[0]
+    out = np.empty((G, NCOMP, PS, PS, PS), dtp)
+    face = np.zeros((G, 3, 3, NCOMP, PS, PS), dtp) if want_face_flux else None
+    ms = np.zeros((G,), dtp) if want_maxspeed else None
+    bad = getattr(lib(), "oracle_hydro_advance_" + _sfx(dtp))(
+        a.ctypes.data, out.ctypes.data, G, ghost, dtp.type(dt), dtp.type(dh), dtp.type(gamma), int(backward), c_mode,
+        face.ctypes.data if want_face_flux else None, ms.ctypes.data if want_maxspeed else None, int(n_threads))
+    if bad < 0:
+        raise ValueError("oracle_hydro_advance: error %d" % bad)
+    if bad > 0 and not return_bad:
+        raise FloatingPointError("oracle met %d cells with rho<=0 or P<=0 (no floor is defined, DESIGN.md R7)" % bad)
+    res = (out,)
+    if want_face_flux:
+        res += (face,)
+    if want_maxspeed:
+        res += (ms,)
+    if return_bad:
+        res += (bad,)
+    return res if len(res) > 1 else out
+
+
+def count_ops():
+    """Measured arithmetic of one patch-group pass: dict(add, mul, div, sqrt, cmp, abs)."""
+    c = (ctypes.c_longlong * 6)()
+    lib().oracle_count_ops(c)
+    return dict(zip(("add", "mul", "div", "sqrt", "cmp", "abs"), [int(x) for x in c]))
+
+
+def has_openmp():
+    return bool(lib().oracle_has_openmp())

@@ -1,0 +1,528 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA code).
+
+Each test states what it pins and which plausible mistake it would catch.  Citations are PAPER.md lines.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import riemann_exact
+from paper_0907_3390_b200 import workloads as W
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+G53 = 5.0 / 3.0
+
+
+def euler_flux(u, gamma):
+    """Physical 1-D Euler flux of u=(rho, m_n, m_t1, m_t2, e) (Eqs.1-3 restricted to one direction), float64."""
+    rho, mn, mt1, mt2, e = u
+    v = mn / rho
+    P = (gamma - 1) * (e - 0.5 * (mn * mn + mt1 * mt1 + mt2 * mt2) / rho)
+    return np.array([mn, mn * v + P, mt1 * v, mt2 * v, (e + P) * v])
+
+
+def random_row(rng, N, gamma, amp=0.2):
+    rho = 1 + amp * rng.uniform(-1, 1, N)
+    v = amp * rng.normal(0, 1, (3, N))
+    P = 1 + amp * rng.uniform(-1, 1, N)
+    return W.conserved(rho, v[0], v[1], v[2], P, gamma)
+
+
+# ------------------------------------------------------------------------------------------------ Eq.11
+def test_van_leer_values_and_symmetry():
+    """Eq.11 (:152-157): harmonic mean for same sign, 0 otherwise.  Catches a dropped factor 2, a wrong sign test."""
+    assert oracle.van_leer(1.0, 3.0) == pytest.approx(1.5, rel=1e-15)      # 2*1*3/(1+3)
+    assert oracle.van_leer(-1.0, -3.0) == pytest.approx(-1.5, rel=1e-15)
+    assert oracle.van_leer(2.0, 2.0) == 2.0                                 # phi(a,a)=a  -> central flux
+    assert oracle.van_leer(1.0, -3.0) == 0.0
+    assert oracle.van_leer(0.0, 5.0) == 0.0
+    assert oracle.van_leer(0.0, 0.0) == 0.0                                 # 0/0 must be a select (R6)
+    rng = np.random.default_rng(1)
+    for a, b in rng.normal(size=(200, 2)):
+        p = oracle.van_leer(a, b)
+        assert p == oracle.van_leer(b, a)
+        assert abs(p) <= 2 * min(abs(a), abs(b)) + 1e-15                    # TVD region
+        if a * b > 0:
+            assert min(a, b) - 1e-15 <= p <= max(a, b) + 1e-15              # harmonic mean lies between
+    assert oracle.van_leer(1e-30, 1e-30, np.float32) == 0.0                 # fp32 product underflow -> 0 (R6)
+
+
+# ------------------------------------------------------------------------------------------------ Eq.8
+def test_cell_fluxes_split_identities():
+    """Eq.8 (:138): F^R - F^L = F(u) (physical flux), F^R + F^L = c u, c = |v_n| + sqrt(gamma P/rho) (:130).
+    Catches a swapped R/L, a missing 1/2, a wrong pressure or energy flux."""
+    rng = np.random.default_rng(2)
+    for _ in range(50):
+        u = random_row(rng, 1, G53, 0.4)[:, 0]
+        FR, FL, c = oracle.cell_fluxes(u, G53)
+        F = euler_flux(u, G53)
+        np.testing.assert_allclose(FR - FL, F, rtol=1e-13, atol=1e-14)
+        np.testing.assert_allclose(FR + FL, c * u, rtol=1e-13, atol=1e-14)
+        rho, mn = u[0], u[1]
+        P = (G53 - 1) * (u[4] - 0.5 * (u[1] ** 2 + u[2] ** 2 + u[3] ** 2) / rho)
+        assert c == pytest.approx(abs(mn / rho) + np.sqrt(G53 * P / rho), rel=1e-14)
+
+
+def test_cell_fluxes_worked_cell():
+    """A cell worked by hand: rho=2, v=(3,0,0), P=4, gamma=2  ->  c_s=2, c=5, e=4/(2-1)+0.5*2*9=13,
+    F=(6, 22, 0, 0, 51), c u=(10, 30, 0, 0, 65): F^R=(8, 26, 0, 0, 58), F^L=(2, 4, 0, 0, 7)."""
+    FR, FL, c = oracle.cell_fluxes(np.array([2.0, 6.0, 0.0, 0.0, 13.0]), 2.0)
+    assert c == 5.0
+    np.testing.assert_allclose(FR, [8.0, 26.0, 0.0, 0.0, 58.0], rtol=1e-15, atol=0)     # w = F/c rounds (22/5, 51/5)
+    np.testing.assert_allclose(FL, [2.0, 4.0, 0.0, 0.0, 7.0], rtol=1e-15, atol=0)
+    # the alternative reading of c (full |v|, R1) differs as soon as there is a transverse velocity
+    _, _, c0 = oracle.cell_fluxes(np.array([2.0, 6.0, 8.0, 0.0, 29.0]), 2.0, c_mode=0)    # v=(3,4,0), P=4
+    _, _, c1 = oracle.cell_fluxes(np.array([2.0, 6.0, 8.0, 0.0, 29.0]), 2.0, c_mode=1)
+    assert c0 == 5.0 and c1 == 7.0
+
+
+# ------------------------------------------------------------------------------------------------ Eq.13
+def test_half_step_is_local_lax_friedrichs():
+    """P-Rusanov: Eqs.8+13 (:138, :168) imply  u^{t+dt/2}_n = u_n - (k/2)[ (F_{n+1}-F_{n-1})/2
+    - (c_{n+1}u_{n+1} - 2 c_n u_n + c_{n-1}u_{n-1})/2 ].  Catches a wrong upwind direction or index in step (b)/(c)."""
+    rng = np.random.default_rng(3)
+    N, k = 12, 0.35
+    u = random_row(rng, N, G53, 0.3)
+    _, uh = oracle.row_update(u, k, G53, want_half=True)
+    F = np.stack([euler_flux(u[:, n], G53) for n in range(N)], axis=1)
+    c = np.array([oracle.cell_fluxes(u[:, n], G53)[2] for n in range(N)])
+    cu = c[None, :] * u
+    for n in range(1, N - 1):
+        llf = u[:, n] - 0.5 * k * (0.5 * (F[:, n + 1] - F[:, n - 1]) - 0.5 * (cu[:, n + 1] - 2 * cu[:, n] + cu[:, n - 1]))
+        np.testing.assert_allclose(uh[:, n], llf, rtol=1e-12, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------------ Eqs.9-12, 14
+def test_full_step_is_conservative_flux_difference():
+    """Eq.14 (:172): u' - u = -k (F_{n+1/2} - F_{n-1/2}) with the returned time-centred fluxes; with the limiter
+    off those are the first-order fluxes of the midpoint state, F^R_n - F^L_{n+1} (:143)."""
+    rng = np.random.default_rng(4)
+    N, k = 16, 0.3
+    u = random_row(rng, N, 1.4, 0.3)
+    for lim in (0, 1):
+        un, uh, fh = oracle.row_update(u, k, 1.4, limiter_on=lim, want_half=True, want_flux=True)
+        for n in range(3, N - 3):
+            np.testing.assert_allclose(un[:, n] - u[:, n], -k * (fh[:, n] - fh[:, n - 1]), rtol=1e-11, atol=1e-13)
+        np.testing.assert_array_equal(un[:, :3], u[:, :3])
+        np.testing.assert_array_equal(un[:, N - 3:], u[:, N - 3:])
+        if lim == 0:
+            for n in range(2, N - 3):
+                FRn, _, _ = oracle.cell_fluxes(uh[:, n], 1.4)
+                _, FLn1, _ = oracle.cell_fluxes(uh[:, n + 1], 1.4)
+                np.testing.assert_allclose(fh[:, n], FRn - FLn1, rtol=1e-13, atol=1e-14)
+
+
+def test_limited_flux_brackets_upwind_and_downwind_values():
+    """Eqs.9-12: where F^R is monotone, F^R_{n+1/2} lies between F^R_n and F^R_{n+1}; at a local extremum of F^R_n
+    no correction is applied (:159).  Stated on the total flux through the returned F_{n+1/2} and cell_fluxes."""
+    rng = np.random.default_rng(5)
+    N, k = 40, 0.2
+    u = random_row(rng, N, G53, 0.3)
+    _, uh, fh = oracle.row_update(u, k, G53, want_half=True, want_flux=True)
+    FR = np.zeros((5, N))
+    FL = np.zeros((5, N))
+    for n in range(1, N - 1):
+        FR[:, n], FL[:, n], _ = oracle.cell_fluxes(uh[:, n], G53)
+    for n in range(2, N - 3):
+        for q in range(5):
+            lo = min(FR[q, n], FR[q, n + 1]) - max(FL[q, n], FL[q, n + 1])
+            hi = max(FR[q, n], FR[q, n + 1]) - min(FL[q, n], FL[q, n + 1])
+            assert lo - 1e-12 <= fh[q, n] <= hi + 1e-12
+            r_ext = (FR[q, n] - FR[q, n - 1]) * (FR[q, n + 1] - FR[q, n]) <= 0
+            l_ext = (FL[q, n + 1] - FL[q, n + 2]) * (FL[q, n] - FL[q, n + 1]) <= 0
+            if r_ext and l_ext:
+                assert fh[q, n] == FR[q, n] - FL[q, n + 1]
+
+
+def test_linear_flux_profile_gives_central_flux():
+    """P-linear: where the cell-centred F^R (and F^L) vary linearly, phi(d,d)=d and Eqs.10-12 give the arithmetic mean
+    of the two neighbours.  Built on the density component with u = const velocity, const P: F^R_rho = rho (c+v)/2 is
+    linear in n when rho is linear and c is constant; c is constant only if c_s is, so use the limiter's defining
+    property on a row where rho, P scale together (c_s const) and v = 0 at the midpoint is not guaranteed —
+    instead check the scale-free statement directly through van_leer."""
+    for d in (0.3, -2.0, 1e-3):
+        a = 1.7
+        assert a + oracle.van_leer(d / 2, d / 2) == pytest.approx(0.5 * (a + (a + d)), rel=1e-15)
+
+
+# ------------------------------------------------------------------------------------------------ :178
+def test_seven_point_stencil():
+    """:178 — the update of cell n depends on cells n-3..n+3 and on nothing farther.  Catches off-by-one ranges."""
+    rng = np.random.default_rng(6)
+    N, k = 21, 0.3
+    u = random_row(rng, N, G53, 0.2)
+    base = oracle.row_update(u, k, G53)
+    n0 = 10
+    for dist in (-4, -3, 3, 4):
+        up = u.copy()
+        up[0, n0 + dist] *= 1.05
+        up[4, n0 + dist] *= 1.05
+        pert = oracle.row_update(up, k, G53)
+        changed = np.any(pert[:, n0] != base[:, n0])
+        assert changed == (abs(dist) <= 3), dist
+
+
+# ------------------------------------------------------------------------------------------------ 3-D invariants
+def _group_batch(seed, G=2, amp=0.2, gamma=G53):
+    rng = np.random.default_rng(seed)
+    shp = (G, 22, 22, 22)
+    rho = 1 + amp * rng.uniform(-1, 1, shp)
+    v = amp * rng.normal(0, 1, (3,) + shp)
+    P = 1 + amp * rng.uniform(-1, 1, shp)
+    u = W.conserved(rho, v[0], v[1], v[2], P, gamma)       # [5][G]...
+    return np.ascontiguousarray(np.moveaxis(u, 0, 1))
+
+
+@pytest.mark.parametrize("backward", [0, 1])
+def test_uniform_state_is_returned_bit_exactly(backward):
+    """P-uniform: equal neighbours -> all flux differences are exactly 0, phi(0,0)=0 -> u unchanged bit for bit."""
+    u = np.empty((1, 5, 22, 22, 22), np.float32)
+    vals = np.array([1.3, 0.4, -0.2, 0.7, 2.9], np.float32)
+    for i in range(5):
+        u[0, i] = vals[i]
+    out = oracle.hydro_advance(u, 0.002, 1 / 128, G53, backward=backward)
+    for i in range(5):
+        assert (out[0, i] == vals[i]).all()
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_mirror_symmetry(axis, dtype):
+    """P-mirror: reflecting the input along an axis and negating that momentum gives the reflected output with that
+    momentum negated.  Pins the 'derived in a similar way' left-moving flux (:141, :164; reading R4)."""
+    u = _group_batch(7).astype(dtype)
+    dt, dh = 0.001, 1 / 128
+    out = oracle.hydro_advance(u, dt, dh, G53)
+    npax = 4 - axis                        # [G][v][z][y][x]
+    um = np.flip(u, axis=npax).copy()
+    um[:, 1 + axis] *= -1
+    outm = oracle.hydro_advance(um, dt, dh, G53)
+    back = np.flip(outm, axis=npax).copy()
+    back[:, 1 + axis] *= -1
+    tol = 4e-6 if dtype == np.float32 else 1e-14
+    np.testing.assert_allclose(back, out, rtol=tol, atol=tol)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_axis_swap_with_backward_flag(dtype):
+    """P-swap: swapping x<->z in the data (and m_x<->m_z) and sweeping backward (z,y,x) is the forward (x,y,z) pass
+    of the original, swapped.  Pins the sweep order flag (:174-176, :326) and the per-sweep component mapping."""
+    u = _group_batch(8).astype(dtype)
+    dt, dh = 0.001, 1 / 128
+    out_f = oracle.hydro_advance(u, dt, dh, G53, backward=0)
+    us = np.ascontiguousarray(np.swapaxes(u, 2, 4))[:, [0, 3, 2, 1, 4]]
+    out_b = oracle.hydro_advance(np.ascontiguousarray(us), dt, dh, G53, backward=1)
+    back = np.ascontiguousarray(np.swapaxes(out_b, 2, 4))[:, [0, 3, 2, 1, 4]]
+    tol = 4e-6 if dtype == np.float32 else 1e-14
+    np.testing.assert_allclose(back, out_f, rtol=tol, atol=tol)
+    # and the order matters: forward != backward on the same data (splitting error), so the flag is not a no-op
+    out_b_same = oracle.hydro_advance(u, dt, dh, G53, backward=1)
+    assert np.abs(out_b_same - out_f).max() > 1e-7
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_one_dimensional_data_reduces_to_the_row_update(axis):
+    """P-1D: for data varying along one axis only with zero transverse momentum the two transverse sweeps are exact
+    no-ops and the 3-D pass equals the 1-D row update replicated, bit for bit (fp32)."""
+    rng = np.random.default_rng(9)
+    row = random_row(rng, 22, 1.4, 0.3)
+    row[2:4] = 0.0
+    row[4] = 1.0 / 0.4 + 0.5 * row[1] ** 2 / row[0]
+    row = row.astype(np.float32)
+    k_dt, dh = np.float32(0.002), np.float32(1 / 128)
+    u = np.zeros((1, 5, 22, 22, 22), np.float32)
+    shape = [1, 1, 1]
+    shape[2 - axis] = 22
+    u[0, 0] = row[0].reshape(shape)
+    u[0, 1 + axis] = row[1].reshape(shape)
+    u[0, 4] = row[4].reshape(shape)
+    out = oracle.hydro_advance(u, k_dt, dh, 1.4)
+    ref = oracle.row_update(row, np.float32(k_dt / dh), 1.4, dtype=np.float32)[:, 3:19]
+    sl = [0, 0, 0]
+    for a in range(16):
+        for b in range(16):
+            idx = [a, b]
+            sel = []
+            for ax_np in range(3):              # numpy axes z,y,x
+                sel.append(slice(None) if ax_np == 2 - axis else idx.pop(0))
+            np.testing.assert_array_equal(out[0, 0][tuple(sel)], ref[0])
+            np.testing.assert_array_equal(out[0, 1 + axis][tuple(sel)], ref[1])
+            np.testing.assert_array_equal(out[0, 4][tuple(sel)], ref[4])
+    for t in range(3):
+        if t != axis:
+            assert (out[0, 1 + t] == 0).all()
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-6), (np.float64, 1e-13)])
+@pytest.mark.parametrize("backward", [0, 1])
+def test_conservation_on_a_periodic_box(dtype, tol, backward):
+    """P-conserve: groups tiled into a periodic box with sibling-copied ghosts: total mass, momentum and energy over
+    all interiors are unchanged by one pass (adjacent groups compute the shared interface flux identically)."""
+    c = W.config1()
+    inp = c["inp"].astype(dtype)
+    out = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward)
+    before = inp[:, :, 3:19, 3:19, 3:19].astype(np.float64)
+    after = out.astype(np.float64)
+    for v in range(5):
+        s0, s1 = before[:, v].sum(), after[:, v].sum()
+        denom = np.abs(before[:, v]).sum()
+        assert abs(s1 - s0) / denom < tol, (v, s0, s1)
+
+
+def test_face_fluxes_account_for_the_interior_change():
+    """:340, :344-346 — the fluxes through the group's outer faces, as output, explain the change of the interior
+    totals: sum(out - in) = -k sum_d sum_faces (F_hi - F_lo).  The mid-plane flux explains each 8-cell patch layer of
+    the last sweep.  Catches a wrong plane index, a wrong variable mapping or transverse index order."""
+    c = W.config1()
+    inp = c["inp"].astype(np.float64)
+    k = c["dt"] / c["dh"]
+    out, face = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], want_face_flux=True)
+    change = (out - inp[:, :, 3:19, 3:19, 3:19]).sum(axis=(2, 3, 4))             # [G][5]
+    net = (face[:, :, 2] - face[:, :, 0]).sum(axis=(1, 3, 4))                     # [G][5]
+    np.testing.assert_allclose(change, -k * net, rtol=1e-9, atol=1e-10)
+    # last sweep (z, forward): lower patch layer k=0..7 changes by -k (F_mid - F_lo) relative to the state before the
+    # z sweep; check through the transverse index order instead: face z is indexed [j][i] like out[v][k][j][i]
+    out_b, face_b = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], backward=1, want_face_flux=True)
+    # backward pass: x is the last sweep; rebuild the pre-x-sweep interior column sums from the x faces [k][j]
+    dx_lo = -(k) * (face_b[:, 0, 1] - face_b[:, 0, 0])                            # [G][5][k][j] change of sum_{i<8}
+    dx_hi = -(k) * (face_b[:, 0, 2] - face_b[:, 0, 1])
+    tot = out_b.sum(axis=4)                                                       # [G][5][k][j]
+    lo, hi = out_b[..., :8].sum(axis=4), out_b[..., 8:].sum(axis=4)
+    # total over i before the x sweep = tot - (dx_lo + dx_hi); it must be the same whether rebuilt from halves
+    np.testing.assert_allclose((lo - dx_lo) + (hi - dx_hi), tot - (dx_lo + dx_hi), rtol=1e-12, atol=1e-12)
+    # forward z-sweep layer statement against an independent route: advance with x,y only is not exposed, so use
+    # mirror: reflecting z swaps the roles of planes 0 and 2 and negates the mass flux through them
+    um = np.flip(inp, axis=2).copy()
+    um[:, 3] *= -1
+    _, face_m = oracle.hydro_advance(um, c["dt"], c["dh"], c["gamma"], want_face_flux=True)
+    np.testing.assert_allclose(face_m[:, 2, 0, 0], -face[:, 2, 2, 0], rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(face_m[:, 2, 1, 0], -face[:, 2, 1, 0], rtol=1e-10, atol=1e-12)
+
+
+def test_group_max_speed_is_eq30_on_the_updated_interior():
+    """:418-426, Eq.30 — one float per group: max over the updated 16^3 cells of c_s + max_i |v_i|."""
+    c = W.config1()
+    inp = c["inp"].astype(np.float64)
+    out, ms = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], want_maxspeed=True)
+    for g in range(out.shape[0]):
+        assert ms[g] == pytest.approx(W.max_signal_speed(out[g], c["gamma"]), rel=1e-14)
+
+
+# ------------------------------------------------------------------------------------------------ precision
+@pytest.mark.parametrize("cfg", ["config1", "config3s"])
+def test_fp32_oracle_tracks_fp64_oracle(cfg):
+    """P-fp: the scheme is well conditioned in fp32 on the workloads: fp32 vs fp64 oracle <= 1e-4 (metric R11)."""
+    if cfg == "config1":
+        c = W.config1()
+        inp = c["inp"]
+    else:
+        c = W.config3()
+        inp = c["inp"][::16]
+    o32 = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], n_threads=4)
+    o64 = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64, n_threads=4)
+    err = W.parity_error(o32, o64, c["gamma"])
+    assert err["max_rel"] < 1e-4, err
+
+
+# ------------------------------------------------------------------------------------------------ Sod
+def _read_golden(name):
+    vals = {}
+    with open(os.path.join(GOLDEN, name)) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            kk, vv = line.split()
+            vals[kk] = float(vv)
+    return vals
+
+
+def test_exact_riemann_solver_matches_textbook_star_values():
+    g = _read_golden("sod_star_region.txt")
+    p, u = riemann_exact.star_state(1, 0, 1, 0.125, 0, 0.1, g["gamma"])
+    assert p == pytest.approx(g["p_star"], abs=6e-6)
+    assert u == pytest.approx(g["u_star"], abs=6e-6)
+    rho, _, _ = riemann_exact.sample(np.array([0.5, 1.2]), 1, 0, 1, 0.125, 0, 0.1, g["gamma"])
+    assert rho[0] == pytest.approx(g["rho_star_L"], abs=6e-6)
+    assert rho[1] == pytest.approx(g["rho_star_R"], abs=6e-6)
+
+
+def sod_chain_1d(gamma, n=128, steps=100, dtype=np.float64, cfl=0.5):
+    """Free-running 1-D Sod run with the oracle's row update, Dirichlet ghosts, dt from Eq.30 each step."""
+    left, right = W.sod_states(gamma)
+    dh = 1.0 / n
+    u = np.empty((5, n + 6), np.float64)
+    x_is_left = (np.arange(n + 6) - 3) < n // 2
+    for v in range(5):
+        u[v] = np.where(x_is_left, left[v], right[v])
+    u = u.astype(dtype)
+    t = 0.0
+    for _ in range(steps):
+        dt = W.cfl_dt(u[:, None].astype(np.float64).reshape(5, -1), dh, gamma, cfl)
+        un = oracle.row_update(u, dt / dh, gamma, dtype=dtype)
+        u[:, 3:-3] = un[:, 3:-3]
+        t += dt
+    return u[:, 3:-3].astype(np.float64), t, dh
+
+
+@pytest.mark.parametrize("gamma", [1.4, G53])
+def test_sod_against_exact_riemann_solution(gamma):
+    """P-Sod (:460-482): 128 cells, 100 steps at CFL 0.5.  L1(rho) against the exact solution <= 1e-2 (Eq.31 form);
+    no new extrema (TVD); velocity and pressure flat across the contact; shock spread over a few cells;
+    Rankine-Hugoniot: the captured post-shock plateau matches the exact star state."""
+    u, t, dh = sod_chain_1d(gamma)
+    n = u.shape[1]
+    x = (np.arange(n) + 0.5) * dh
+    rho_e, v_e, p_e = riemann_exact.sample((x - 0.5) / t, 1, 0, 1, 0.125, 0, 0.1, gamma)
+    rho = u[0]
+    v = u[1] / u[0]
+    P = (gamma - 1) * (u[4] - 0.5 * u[1] ** 2 / u[0])
+    l1 = np.mean(np.abs(rho - rho_e))
+    assert l1 <= 1.0e-2, l1
+    assert rho.max() <= 1.0 + 1e-12 and rho.min() >= 0.125 - 1e-12             # no new extrema
+    # away from the contact and the shock the error stays within the 1-3 % the paper reports for the rarefaction
+    # (:482); component-wise limiting of a system is not strictly monotone, so a small start-up dip at the
+    # rarefaction tail is part of the method (it is there in the paper's Fig.13 too) and is bounded, not forbidden
+    ps0, us0 = riemann_exact.star_state(1, 0, 1, 0.125, 0, 0.1, gamma)
+    a_r = np.sqrt(gamma * 0.1 / 0.125)
+    gp, gm = gamma + 1, gamma - 1
+    x_shock = 0.5 + t * a_r * np.sqrt(gp / (2 * gamma) * ps0 / 0.1 + gm / (2 * gamma))
+    x_contact = 0.5 + us0 * t
+    smooth = (np.abs(x - x_shock) > 6 * dh) & (np.abs(x - x_contact) > 8 * dh)
+    # measured: 5.5 % (gamma=1.4) / 4.9 % (5/3) at the rounded rarefaction tail with 128 cells, halving with the cell
+    # size (3.5 -> 2.0 -> 1.0 % inside the fan at 128/256/512 cells), i.e. the paper's 1-3 % at its finer grid
+    assert (np.abs(rho - rho_e) / rho_e)[smooth].max() < 0.06
+    u2, t2, dh2 = sod_chain_1d(gamma, n=256, steps=200)
+    x2 = (np.arange(256) + 0.5) * dh2
+    rho_e2, _, _ = riemann_exact.sample((x2 - 0.5) / t2, 1, 0, 1, 0.125, 0, 0.1, gamma)
+    l1_2 = np.mean(np.abs(u2[0] - rho_e2))
+    assert 0.4 < l1_2 / l1 < 0.65, (l1, l1_2)          # first-order L1 convergence with discontinuities present
+    ps, us = riemann_exact.star_state(1, 0, 1, 0.125, 0, 0.1, gamma)
+    xc = 0.5 + us * t                                                           # contact position
+    near = np.abs(x - xc) < 4 * dh
+    assert np.abs(v[near] - us).max() < 0.02 * us                               # v, P uniform across the contact
+    assert np.abs(P[near] - ps).max() < 0.02 * ps
+    # shock: number of cells between 5 % and 95 % of the density jump
+    rs = rho_e[(x > xc + 3 * dh)].max()
+    frac = (rho - 0.125) / (rs - 0.125)
+    right_of_contact = x > xc + 6 * dh
+    width = np.sum((frac > 0.05) & (frac < 0.95) & right_of_contact)
+    assert 1 <= width <= 5, width
+
+
+SOD_L1_FP64 = {}
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_sod_3d_pass_equals_1d_chain_along_each_axis(axis):
+    """Config 2 geometry, reduced across (128 x 16 x 16 = 8 groups): the 3-D pass along each axis, free-running for
+    10 steps in fp32 with ghost refill, is bit-identical to the 1-D chain (transverse sweeps are exact no-ops)."""
+    gamma = 1.4
+    U, left, right = W.config2_box(axis, gamma, 128, 16)
+    U = U.astype(np.float32)
+    dh = 1.0 / 128
+    shp = U.shape[1:]
+    grid = (shp[0] // 16, shp[1] // 16, shp[2] // 16)
+    # 1-D chain in fp32 with the same dt sequence
+    line = np.empty((5, 134), np.float32)
+    sel = [0, 0, 0]
+    sel[2 - axis] = slice(None)
+    for v in range(5):
+        line[v, 3:-3] = U[(v,) + tuple(sel)]
+        line[v, :3] = np.float32(left[v])
+        line[v, -3:] = np.float32(right[v])
+    line = line[[0, 1 + axis, 1 + (axis + 1) % 3, 1 + (axis + 2) % 3, 4]]
+    for _ in range(10):
+        inp = W.box_to_groups(U, dirichlet_axis=axis, lo_state=left.astype(np.float32), hi_state=right.astype(np.float32))
+        dt = W.cfl_dt(inp, dh, gamma)
+        out = oracle.hydro_advance(inp, dt, dh, gamma, n_threads=4)
+        U = W.groups_to_box(out, grid)
+        ln = oracle.row_update(line, np.float32(np.float32(dt) / np.float32(dh)), gamma, dtype=np.float32)
+        line[:, 3:-3] = ln[:, 3:-3]
+    np.testing.assert_array_equal(U[(0,) + tuple(sel)], line[0, 3:-3])
+    np.testing.assert_array_equal(U[(1 + axis,) + tuple(sel)], line[1, 3:-3])
+    np.testing.assert_array_equal(U[(4,) + tuple(sel)], line[4, 3:-3])
+    assert (U[0] == U[(0,) + tuple(sel)].reshape([128 if a == 2 - axis else 1 for a in range(3)])).all()
+
+
+# ------------------------------------------------------------------------------------------------ order of accuracy
+def _acoustic_l1(n, v0, gamma=G53, amp=1e-6):
+    """1-D travelling sound wave (:450-458: rho0=1, P0=3/5, gamma=5/3 -> c_s=1) on a uniform flow v0, periodic,
+    one period, fp64.  Returns L1(rho)/amp (Eq.31 form)."""
+    rho0, P0 = 1.0, 3.0 / 5.0
+    cs = np.sqrt(gamma * P0 / rho0)
+    dh = 1.0 / n
+    x = (np.arange(n) + 0.5) * dh
+
+    def state(xx):
+        d = amp * np.sin(2 * np.pi * xx)
+        return W.conserved(rho0 * (1 + d), v0 + cs * d, 0 * xx, 0 * xx, P0 * (1 + gamma * d), gamma)
+
+    u = state(x)
+    t_end = 1.0 / (cs + v0)
+    nsteps = int(np.ceil(t_end / (0.5 * dh / (cs + abs(v0) + 1e-5))))
+    dt = t_end / nsteps
+    for _ in range(nsteps):
+        up = np.concatenate([u[:, -3:], u, u[:, :3]], axis=1)
+        u = oracle.row_update(up, dt / dh, gamma)[:, 3:-3]
+    return np.mean(np.abs(u[0] - state(x)[0])) / amp
+
+
+def test_second_order_convergence_on_a_sound_wave():
+    """P-order (:450-458): the L1 error of a small-amplitude sound wave converges at second order.  On a uniform flow
+    (v0 = 0.5, so that v never changes sign) the slope is -2.0 (window [-2.25, -1.85]); the paper reports -1.9 and
+    blames points where the solver drops to first order.  With the gas at rest on average (v0 = 0) the freezing
+    speed |v| + c_s has a kink at every velocity node and the measured slope is -1.5 (window [-1.7, -1.25]) — same
+    with or without the limiter (reading R20).  Catches any mistake that degrades Eqs.9-14 to first order
+    (slope -1) or makes them unstable."""
+    errs = [_acoustic_l1(n, 0.5) for n in (32, 64, 128, 256)]
+    slopes = [np.log2(errs[i + 1] / errs[i]) for i in range(3)]
+    assert all(-2.25 <= s <= -1.85 for s in slopes), (errs, slopes)
+    errs0 = [_acoustic_l1(n, 0.0) for n in (32, 64, 128)]
+    slopes0 = [np.log2(errs0[i + 1] / errs0[i]) for i in range(2)]
+    assert all(-1.7 <= s <= -1.25 for s in slopes0), (errs0, slopes0)
+
+
+def test_second_order_convergence_3d_diagonal_wave_strang_pair():
+    """:174-176, :452 — a sound wave along the box diagonal (the paper's K = (1,1,1)/sqrt 3) on a uniform diagonal
+    flow, advanced by forward+backward pairs with the same dt on 16^3 and 32^3 periodic boxes (fp64): the error falls
+    by more than first order.  Pins the 3-D splitting, the transverse-momentum fluxes and the backward flag together."""
+    gamma, amp = G53, 1e-6
+    rho0, P0, cs, vb = 1.0, 3.0 / 5.0, 1.0, 0.3
+    speed = cs + np.sqrt(3.0) * vb               # phase speed along the diagonal
+
+    def run(n):
+        dh = 1.0 / n
+        c = (np.arange(n) + 0.5) * dh
+        Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+
+        def state(shift):
+            d = amp * np.sin(2 * np.pi * (X + Y + Z - shift))
+            vc = vb + cs * d / np.sqrt(3.0)
+            return W.conserved(rho0 * (1 + d), vc, vc, vc, P0 * (1 + gamma * d), gamma)
+
+        U = state(0.0)
+        grid = (n // 16,) * 3
+        t_end = 1.0 / (np.sqrt(3.0) * speed)     # one period: wavelength 1/sqrt 3 along the diagonal
+        nsteps = int(np.ceil(t_end / (0.4 * dh / (cs / np.sqrt(3.0) * 0 + cs + vb))))
+        nsteps += nsteps % 2
+        dt = t_end / nsteps
+        for s in range(nsteps):
+            inp = W.box_to_groups(U)
+            out = oracle.hydro_advance(inp, dt, dh, gamma, backward=s % 2, n_threads=8)
+            U = W.groups_to_box(out, grid)
+        return np.mean(np.abs(U[0] - state(np.sqrt(3.0) * speed * t_end)[0])) / amp
+
+    e16, e32 = run(16), run(32)
+    slope = np.log2(e32 / e16)
+    assert -2.6 <= slope <= -1.5, (e16, e32, slope)
+
+
+def test_op_count_is_stable():
+    """The measured arithmetic of one group pass (DESIGN.md §Roofline uses it): rows = 22*22 + 16*22 + 16*16 = 1092,
+    2 sqrt-free cells... the sqrt count is exactly (22 + 20) cells per row."""
+    c = oracle.count_ops()
+    assert c["sqrt"] == 1092 * 42
+    assert c["abs"] == 1092 * 42
+    assert c["cmp"] == 1092 * 17 * 10           # one select per component, family and limited interface
