@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py — hydro cell-updates/s of the batched relaxing-TVD update on B200, with roofline and CPU baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5|4|3]
+
+One "step" = one pass of the whole hot path (H0-H9 of DESIGN.md: stage, three sweeps, store) over one batch:
+one `gamer_hydro_advance` call on the workload.  Default workload = BASELINE.json configs[4] ("config 5": 32 768
+patch groups, 134 M interior cells, 6.98 GB in / 2.68 GB out — the configuration the metric's roofline target is
+quoted on), synthetic, filled on the device.  Inputs are far larger than L2 (126 MB), so every step streams from HBM.
+
+Prints ONE JSON line (rank 0).  `value` = interior cell-updates per second, device-resident inputs, timed with
+CUDA events on the launching stream; `e2e` = the same metric through `gamer_hydro_pipeline_run` with HOST (pinned)
+buffers, host<->device copies inside the timed region.  N > 1 (torchrun): independent replicas, no collective on
+the data path ("replicas only") — each rank advances its own copy of the workload.
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_0907_3390_b200 import workloads as W  # noqa: E402
+
+METRIC = "hydro cell-updates/sec (fp32) on 1 B200; % of roofline (HBM GB/s)"
+UNIT = "cell-updates/s"
+CELLS_PER_GROUP = 16 ** 3
+BYTES_PER_GROUP = 212960 + 81920            # padded in + interior out
+FLOPS_PER_GROUP = 1092 * 3474                # rows x flops per row, FMA = 2
+FP32_LANES_PER_SM = 128
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.sm_max = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        if not self.samples:
+            return dict(sm_mhz=None, sm_max_mhz=self.sm_max, reasons=sorted(self.reasons), samples=0)
+        return dict(sm_mhz=float(np.median(self.samples)), sm_max_mhz=self.sm_max, reasons=sorted(self.reasons),
+                    samples=len(self.samples))
+
+
+def physical_gpu_index(local):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local])
+        except Exception:
+            return local
+    return local
+
+
+def make_device_workload(config, torch, device, n_override=None):
+    """Returns (d_in, n_groups, dt, dh, gamma, description)."""
+    if config == 5:
+        n = n_override or W.CONFIG5["n_groups"]
+        hot = W.config5_hot_groups(n)
+        bg = torch.from_numpy(W.config5_group(False)).to(device)
+        ht = torch.from_numpy(W.config5_group(True)).to(device)
+        d_in = torch.empty((n, 5, 22, 22, 22), dtype=torch.float32, device=device)
+        d_in[:] = bg
+        d_in[torch.from_numpy(hot).to(device)] = ht
+        return d_in, n, W.config5_dt(), W.CONFIG5["dh"], W.CONFIG5["gamma"], \
+            "config5: %d groups, Sedov-like blast seeds in 1%% of groups (rho=1, p=1e-5, hot 2^3 cells p=1e3)" % n
+    c = {4: W.config4, 3: W.config3}[config]()
+    inp = c["inp"] if n_override is None else c["inp"][:n_override]
+    d_in = torch.from_numpy(inp).to(device)
+    return d_in, inp.shape[0], c["dt"], c["dh"], c["gamma"], "%s: %d groups" % (c["name"], inp.shape[0])
+
+
+def cpu_sample(config, n_sample):
+    """A bounded sample of the same workload for the oracle: the first n_sample groups (config 5 keeps its 1 % hot)."""
+    if config == 5:
+        c = W.config5(range(n_sample))
+    else:
+        c = {4: W.config4, 3: W.config3}[config]()
+        c["inp"] = c["inp"][:n_sample]
+    return c
+
+
+def time_oracle(config, cores, target_core_seconds=20.0, n_sample=None):
+    import oracle
+    probe = cpu_sample(config, 32)
+    t0 = time.perf_counter()
+    oracle.hydro_advance(probe["inp"], probe["dt"], probe["dh"], probe["gamma"], n_threads=1, return_bad=True)
+    per_group = (time.perf_counter() - t0) / 32
+    if n_sample is None:
+        n_sample = int(max(8, min(8192, target_core_seconds / per_group)))
+    c = cpu_sample(config, n_sample)
+    n_sample = c["inp"].shape[0]
+    t0 = time.perf_counter()
+    oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"], n_threads=cores, return_bad=True)
+    wall = time.perf_counter() - t0
+    return dict(value=n_sample * CELLS_PER_GROUP / wall, unit=UNIT, cores=cores, kind="oracle",
+                sample="first %d groups of the workload, fp32 oracle, %d OpenMP threads over groups, %.2f s wall"
+                       % (n_sample, cores, wall)), c, wall
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    import oracle
+    # each step is a bounded sample sized so that the whole --steps/--warmup run ends within about two minutes
+    per_step_wall = min(1.5, 120.0 / max(1, args.steps + args.warmup))
+    _, c, _ = time_oracle(args.config, cores, target_core_seconds=per_step_wall * cores)
+    n_sample = c["inp"].shape[0]
+    for _ in range(args.warmup):
+        oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"], n_threads=cores, return_bad=True)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"], n_threads=cores, return_bad=True)
+    wall = time.perf_counter() - t0
+    value = args.steps * n_sample * CELLS_PER_GROUP / wall
+    sample = "each step = first %d groups of the workload (bounded sample), fp32 oracle, %d OpenMP threads" % (n_sample, cores)
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * wall / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f32", data="synthetic", impl="reference",
+                config=dict(workload="config%d" % args.config, sample_groups=n_sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    from paper_0907_3390_b200 import hydro
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+
+    hydro.lib()     # fail loudly here if the CUDA library is missing
+    peaks = load_peaks()
+    d_in, n, dt, dh, gamma, desc = make_device_workload(args.config, torch, device, args.groups)
+    d_out = torch.empty((n, 5, 16, 16, 16), dtype=torch.float32, device=device)
+    info = hydro.gamer_hydro_launch_info(n)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        hydro.gamer_hydro_advance(d_in, d_out, n, 3, dt, dh, gamma, stream=stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(physical_gpu_index(local))
+    sampler.start()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    evs[0].record(stream)
+    for i in range(args.steps):
+        step()
+        evs[i + 1].record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    if dist is not None:
+        dist.barrier()
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per_launch_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
+    if dist is not None:
+        t = torch.tensor([total_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * n * CELLS_PER_GROUP / (ms_per_step * 1e-3)
+    kernel_ms = float(np.mean(per_launch_ms))
+
+    # spot check of the timed output against the oracle (a few groups), so that a wrong-but-fast run cannot pass
+    parity = None
+    if rank == 0 and not args.no_check:
+        import oracle
+        idx = np.unique(np.concatenate([W.config5_hot_groups(n)[:3], [0, n - 1]])) if args.config == 5 \
+            else np.array([0, n // 2, n - 1])
+        sub = d_in[torch.from_numpy(idx).to(device)].cpu().numpy()
+        ref = oracle.hydro_advance(sub, dt, dh, gamma, n_threads=1, return_bad=True)[0]
+        got = d_out[torch.from_numpy(idx).to(device)].cpu().numpy()
+        parity = W.parity_error(got, ref, gamma)["max_rel"]
+
+    # roofline of the one kernel of the step
+    n_sm = torch.cuda.get_device_properties(device).multi_processor_count
+    fp32_peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    ach_gbs = n * BYTES_PER_GROUP / (kernel_ms * 1e-3) / 1e9
+    ach_tf = n * FLOPS_PER_GROUP / (kernel_ms * 1e-3) / 1e12
+    roofline_hbm = dict(bound="hbm", achieved=ach_gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach_gbs / peaks["hbm_gbs"],
+                        traffic=None, peak_source=peaks["source"])
+    roofline_alu = dict(bound="alu", achieved=ach_tf, peak=fp32_peak_tflops, unit="TFLOP/s", frac=ach_tf / fp32_peak_tflops,
+                        traffic=None, peak_source="derived: %d SM x 128 FP32 lanes x 2 x sm_max_mhz (DESIGN.md)" % n_sm)
+    # the metric's roofline is the slower of the two bounds (north_star): FP32 at 51 ns/group vs HBM at 45 ns/group
+    t_alu = FLOPS_PER_GROUP / (fp32_peak_tflops * 1e12)
+    t_hbm = BYTES_PER_GROUP / (peaks["hbm_gbs"] * 1e9)
+    roofline = dict(roofline_alu if t_alu >= t_hbm else roofline_hbm)
+    roofline["kernel_ms"] = kernel_ms
+    roofline["ns_per_group"] = kernel_ms * 1e6 / n
+
+    # end to end through the public C-ABI call with host buffers
+    e2e = None
+    if rank == 0 or world > 1:
+        try:
+            h_in = torch.empty(d_in.shape, dtype=torch.float32, pin_memory=True)
+            h_out = torch.empty(d_out.shape, dtype=torch.float32, pin_memory=True)
+            h_in.copy_(d_in)
+            torch.cuda.synchronize()
+            e2e_steps = max(1, min(args.steps, args.e2e_steps))
+            chunk, ns = args.chunk, args.streams
+            hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, dt, dh, gamma, 0, chunk, ns)      # warm-up
+            if dist is not None:
+                dist.barrier()
+            t0 = time.perf_counter()
+            for _ in range(e2e_steps):
+                hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, dt, dh, gamma, 0, chunk, ns)
+            wall = time.perf_counter() - t0
+            if dist is not None:
+                t = torch.tensor([wall], device=device, dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                wall = float(t.item())
+            e2e = dict(value=world * e2e_steps * n * CELLS_PER_GROUP / wall, unit=UNIT,
+                       h2d_bytes_per_step=int(h_in.numel() * 4), d2h_bytes_per_step=int(h_out.numel() * 4),
+                       steps=e2e_steps, ms_per_step=1e3 * wall / e2e_steps, groups_per_chunk=chunk, n_streams=ns,
+                       h2d_gbs=h_in.numel() * 4 * e2e_steps / wall / 1e9, api="gamer_hydro_pipeline_run (pinned host)")
+            del h_in, h_out
+        except Exception as ex:      # e.g. not enough pinnable host memory
+            e2e = dict(value=None, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0, error=str(ex)[:200])
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cores = os.cpu_count() or 1
+        cpu_baseline, _, _ = time_oracle(args.config, cores)
+
+    if rank == 0:
+        line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                    ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                    data="synthetic",
+                    config=dict(workload=desc, n_groups=n, cells_per_group=CELLS_PER_GROUP, parallelism="replicas x%d" % world,
+                                l2="inputs (%.2f GB) larger than L2; no flush needed" % (d_in.numel() * 4 / 1e9),
+                                launch=info),
+                    roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
+                    cpu_baseline=cpu_baseline, e2e=e2e, gpu_launches=args.steps, clocks=clocks,
+                    parity_spot_check_max_rel=parity)
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, choices=[3, 4, 5])
+    ap.add_argument("--groups", type=int, default=None, help="debug: override the number of groups")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--chunk", type=int, default=2048, help="pipeline: groups per chunk (N_g)")
+    ap.add_argument("--streams", type=int, default=4, help="pipeline: number of streams (N_s)")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-check", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,104 @@
+/* gamer_hydro.h — C ABI of the batched relaxing-TVD hydrodynamic update of GAMER (arXiv 0907.3390) for B200 (sm_100a).
+ *
+ * The operation ("GPU hydrodynamic solver", §3.1): many independent, fixed-size patch groups are
+ * advanced by one dimensionally split pass (three 1-D sweeps) of the second-order relaxing TVD scheme of PAPER.md
+ * §2.2 (Eqs.6-14, :126-172): first-order upwind half step, van-Leer-limited second-order full step, on the five
+ * conserved variables (rho, rho v_x, rho v_y, rho v_z, e), fp32 (:448).
+ *
+ * LAYOUT (the contract)
+ *   in [g][v][z][y][x]   g slowest, x fastest; v in {0:rho, 1:rho v_x, 2:rho v_y, 3:rho v_z, 4:e};
+ *                        extents 22 = 2*8 + 2*3 in x, y, z (:324): 16 interior cells (two 8-cell patches) plus
+ *                        `ghost` = 3 cells on each side (7-point stencil, :178).  Interior = indices 3..18.
+ *                        212 960 bytes per group.
+ *   out[g][v][k][j][i]   extents 16; out[g][v][k][j][i] is padded cell (k+3, j+3, i+3).  No ghost zones are written
+ *                        (:344).  81 920 bytes per group.
+ *   face_flux[g][d][p][v][b][a]  (optional) time-centred fluxes F^{t+dt/2} of Eq.14 through the three planes normal to
+ *                        axis d (0:x, 1:y, 2:z) that bound the two 8-cell patch layers — padded interfaces 2|3 (p=0),
+ *                        10|11 (p=1), 18|19 (p=2) — on the 16x16 interior transverse cells, (b,a) = the two
+ *                        transverse interior indices, slower first: d=x:(k,j), d=y:(k,i), d=z:(j,i).  These are the
+ *                        "fluxes across the boundaries of each patch" of :340/:344-346.  46 080 bytes per group.
+ *   group_maxspeed[g]    (optional) max over the group's 16^3 UPDATED cells of c_s + max(|v_x|,|v_y|,|v_z|), the
+ *                        denominator of the CFL condition Eq.30 (:418-426: "a single floating-point value per patch
+ *                        group").
+ *
+ * WHAT THE LIBRARY DOES NOT DO: it does not fill ghost zones (the caller's "preparation step", :322), it does not
+ * choose dt (:418-426 — it only offers the per-group reduction), it applies no density or pressure floor (the
+ * paper names none): non-physical input (rho <= 0 or P <= 0) yields NaN/Inf in the affected cells, silently.
+ *
+ * OWNERSHIP: the caller owns every buffer.  `d_*` are DEVICE pointers (cudaMalloc or equivalent) valid on the
+ * device of `stream`; `h_*` are HOST pointers.  Nothing is allocated, freed or synchronised by gamer_hydro_advance*:
+ * they only enqueue work on `stream` (NULL = the legacy default stream).  `d_in` is never written.  Input and output
+ * must not overlap.
+ *
+ * ERRORS: every function returns GAMER_OK (0) or a negative gamer_status; nothing aborts or throws.  After a
+ * failure gamer_last_error() returns a thread-local, statically stored, human-readable message.
+ *   ghost != 3                                                        -> GAMER_EUNSUPPORTED  (stencil, :178)
+ *   n_groups < 0; a required pointer NULL while n_groups > 0; a pointer not 16-byte aligned;
+ *   !(dh > 0); !(dt >= 0); !(gamma > 1); backward not 0/1              -> GAMER_EINVAL
+ *   n_groups == 0                                                     -> GAMER_OK, nothing enqueued
+ *   a CUDA runtime error (launch, attribute, copy)                    -> GAMER_ECUDA
+ *   an allocation failure inside gamer_hydro_pipeline_run             -> GAMER_ENOMEM
+ */
+#ifndef GAMER_HYDRO_H
+#define GAMER_HYDRO_H
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define GAMER_API __attribute__((visibility("default")))
+#else
+#define GAMER_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum gamer_status {
+    GAMER_OK = 0,
+    GAMER_EINVAL = -1,
+    GAMER_EUNSUPPORTED = -2,
+    GAMER_ECUDA = -3,
+    GAMER_ENOMEM = -4
+};
+
+/* One forward pass (sweeps x, then y, then z) over n_groups patch groups, each sweep with the full dt
+ * (Eqs.13-14).  d_in, d_out: device pointers, layouts above.  dt, dh: time step and cell size (only dt/dh enters).
+ * gamma: ratio of specific heats (Eq.5).  stream: a cudaStream_t passed as void*.  Asynchronous. */
+GAMER_API int gamer_hydro_advance(const float* d_in, float* d_out, long long n_groups, int ghost,
+                        float dt, float dh, float gamma, void* stream);
+
+/* Same with the paper's sweep-direction boolean (:326): backward = 0 sweeps x,y,z; backward = 1 sweeps z,y,x.
+ * d_face_flux and d_group_maxspeed are optional device outputs (NULL = not computed), layouts above. */
+GAMER_API int gamer_hydro_advance_ex(const float* d_in, float* d_out, long long n_groups, int ghost,
+                           float dt, float dh, float gamma, int backward,
+                           float* d_face_flux, float* d_group_maxspeed, void* stream);
+
+/* Buffer sizes in floats: n*5*(16+2*ghost)^3, n*5*16^3, n*3*3*5*16*16.  0 if n_groups < 0 or ghost < 0. */
+GAMER_API size_t gamer_hydro_in_floats(long long n_groups, int ghost);
+GAMER_API size_t gamer_hydro_out_floats(long long n_groups);
+GAMER_API size_t gamer_hydro_face_flux_floats(long long n_groups);
+
+/* Secondary subsystem — the stream pipeline of PAPER.md:350-356 / Fig.5: n_groups groups in HOST memory are cut
+ * into chunks of groups_per_chunk (the paper's N_g) that travel round-robin through n_streams (N_s) CUDA streams,
+ * each doing one host->device copy, one kernel, one device->host copy, so that copies overlap kernels of other
+ * chunks.  h_in / h_out: host pointers, same layouts as d_in / d_out; page-locked (pinned) memory is needed for the
+ * copies to overlap — pageable memory works but serialises.  The call allocates and frees its own device staging
+ * buffers (n_streams * groups_per_chunk groups), runs on the current device and is SYNCHRONOUS: on return h_out is
+ * complete.  1 <= n_streams <= 16, groups_per_chunk >= 1, else GAMER_EINVAL. */
+GAMER_API int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups, int ghost,
+                             float dt, float dh, float gamma, int backward,
+                             long long groups_per_chunk, int n_streams);
+
+/* Launch geometry the library will use on the current device, for reporting: any pointer may be NULL.
+ * grid = number of persistent CTAs for n_groups, block = threads per CTA, smem = dynamic shared memory per CTA in
+ * bytes, regs = registers per thread of the kernel. */
+GAMER_API int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread);
+
+GAMER_API const char* gamer_last_error(void);   /* thread-local, static storage; "" if the last call on this thread succeeded */
+GAMER_API const char* gamer_version(void);      /* static string */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GAMER_HYDRO_H */

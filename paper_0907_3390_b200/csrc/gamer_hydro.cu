@@ -1,0 +1,233 @@
+// gamer_hydro.cu — the C ABI of include/gamer_hydro.h: argument validation, launch, and the stream pipeline.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/gamer_hydro.h"
+#include "hydro_kernel.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+using KernelFn = void (*)(const float*, float*, long long, gamer::GasConst, float*, float*);
+
+KernelFn pick_kernel(bool backward, bool face, bool speed) {
+    using namespace gamer;
+    const int key = (backward ? 4 : 0) | (face ? 2 : 0) | (speed ? 1 : 0);
+    switch (key) {
+        case 0: return hydro_advance_kernel<false, false, false>;
+        case 1: return hydro_advance_kernel<false, false, true>;
+        case 2: return hydro_advance_kernel<false, true, false>;
+        case 3: return hydro_advance_kernel<false, true, true>;
+        case 4: return hydro_advance_kernel<true, false, false>;
+        case 5: return hydro_advance_kernel<true, false, true>;
+        case 6: return hydro_advance_kernel<true, true, false>;
+        default: return hydro_advance_kernel<true, true, true>;
+    }
+}
+
+struct DeviceInfo {
+    bool ready = false;
+    int sm_count = 0;
+    bool attr_set[8] = {false, false, false, false, false, false, false, false};
+};
+std::mutex g_mu;
+DeviceInfo g_dev[64];
+
+// SM count of the current device and the opt-in to 208 KB of dynamic shared memory, once per device and kernel.
+int prepare(KernelFn fn, int key, int* sm_count) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= 64) return fail(GAMER_ECUDA, "device ordinal %d out of range", dev);
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceInfo& di = g_dev[dev];
+    if (!di.ready) {
+        int major = 0, smem_optin = 0;
+        e = cudaDeviceGetAttribute(&di.sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+        if (major != 10)
+            return fail(GAMER_EUNSUPPORTED, "this library is built for sm_100a only; device %d has compute capability %d.x",
+                        dev, major);
+        if (smem_optin < gamer::SMEM_BYTES)
+            return fail(GAMER_EUNSUPPORTED, "device offers %d B of shared memory per block, %d needed", smem_optin,
+                        gamer::SMEM_BYTES);
+        di.ready = true;
+    }
+    if (!di.attr_set[key]) {
+        e = cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 gamer::SMEM_BYTES);
+        if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
+        di.attr_set[key] = true;
+    }
+    *sm_count = di.sm_count;
+    return GAMER_OK;
+}
+
+int validate(const void* in, const void* out, long long n_groups, int ghost, float dt, float dh, float gamma,
+             int backward, const void* face, const void* speed) {
+    if (ghost != gamer::NG)
+        return fail(GAMER_EUNSUPPORTED, "ghost = %d: the 7-point stencil of the scheme fixes ghost = 3", ghost);
+    if (n_groups < 0) return fail(GAMER_EINVAL, "n_groups = %lld < 0", n_groups);
+    if (!(dh > 0.f)) return fail(GAMER_EINVAL, "dh must be > 0");
+    if (!(dt >= 0.f)) return fail(GAMER_EINVAL, "dt must be >= 0");
+    if (!(gamma > 1.f)) return fail(GAMER_EINVAL, "gamma must be > 1");
+    if (backward != 0 && backward != 1) return fail(GAMER_EINVAL, "backward must be 0 or 1");
+    if (n_groups > 0 && (in == nullptr || out == nullptr)) return fail(GAMER_EINVAL, "NULL input or output pointer");
+    if (!aligned16(in) || !aligned16(out) || !aligned16(face) || !aligned16(speed))
+        return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
+    return GAMER_OK;
+}
+
+gamer::GasConst make_const(float dt, float dh, float gamma) {
+    gamer::GasConst gc;
+    const float k = dt / dh;
+    gc.gm1 = gamma - 1.0f;
+    gc.ggm1 = gamma * (gamma - 1.0f);
+    gc.kq = 0.25f * k;
+    gc.kh = 0.5f * k;
+    return gc;
+}
+
+int launch(const float* d_in, float* d_out, long long n_groups, float dt, float dh, float gamma, int backward,
+           float* d_face, float* d_speed, cudaStream_t stream) {
+    const int key = (backward ? 4 : 0) | (d_face ? 2 : 0) | (d_speed ? 1 : 0);
+    KernelFn fn = pick_kernel(backward != 0, d_face != nullptr, d_speed != nullptr);
+    int sm_count = 0;
+    const int rc = prepare(fn, key, &sm_count);
+    if (rc != GAMER_OK) return rc;
+    const int grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
+    fn<<<grid, gamer::BLOCK_THREADS, gamer::SMEM_BYTES, stream>>>(d_in, d_out, n_groups, make_const(dt, dh, gamma),
+                                                                  d_face, d_speed);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GAMER_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
+    return GAMER_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gamer_hydro_advance_ex(const float* d_in, float* d_out, long long n_groups, int ghost, float dt, float dh,
+                           float gamma, int backward, float* d_face_flux, float* d_group_maxspeed, void* stream) {
+    const int rc = validate(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward, d_face_flux, d_group_maxspeed);
+    if (rc != GAMER_OK) return rc;
+    g_err[0] = '\0';
+    if (n_groups == 0) return GAMER_OK;
+    return launch(d_in, d_out, n_groups, dt, dh, gamma, backward, d_face_flux, d_group_maxspeed,
+                  static_cast<cudaStream_t>(stream));
+}
+
+int gamer_hydro_advance(const float* d_in, float* d_out, long long n_groups, int ghost, float dt, float dh,
+                        float gamma, void* stream) {
+    return gamer_hydro_advance_ex(d_in, d_out, n_groups, ghost, dt, dh, gamma, 0, nullptr, nullptr, stream);
+}
+
+size_t gamer_hydro_in_floats(long long n_groups, int ghost) {
+    if (n_groups < 0 || ghost < 0) return 0;
+    const size_t n = (size_t)(gamer::PS + 2 * ghost);
+    return (size_t)n_groups * gamer::NCOMP * n * n * n;
+}
+size_t gamer_hydro_out_floats(long long n_groups) {
+    return n_groups < 0 ? 0 : (size_t)n_groups * gamer::GROUP_OUT_FLOATS;
+}
+size_t gamer_hydro_face_flux_floats(long long n_groups) {
+    return n_groups < 0 ? 0 : (size_t)n_groups * gamer::GROUP_FACE_FLOATS;
+}
+
+int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups, int ghost, float dt, float dh,
+                             float gamma, int backward, long long groups_per_chunk, int n_streams) {
+    const int rc = validate(h_in, h_out, n_groups, ghost, dt, dh, gamma, backward, nullptr, nullptr);
+    if (rc != GAMER_OK) return rc;
+    if (n_streams < 1 || n_streams > 16) return fail(GAMER_EINVAL, "n_streams must be in 1..16");
+    if (groups_per_chunk < 1) return fail(GAMER_EINVAL, "groups_per_chunk must be >= 1");
+    g_err[0] = '\0';
+    if (n_groups == 0) return GAMER_OK;
+    if (groups_per_chunk > n_groups) groups_per_chunk = n_groups;
+    const long long n_chunks = (n_groups + groups_per_chunk - 1) / groups_per_chunk;
+    if (n_streams > n_chunks) n_streams = (int)n_chunks;
+
+    const size_t in_bytes = (size_t)groups_per_chunk * gamer::GROUP_IN_FLOATS * sizeof(float);
+    const size_t out_bytes = (size_t)groups_per_chunk * gamer::GROUP_OUT_FLOATS * sizeof(float);
+    std::vector<cudaStream_t> streams((size_t)n_streams, nullptr);
+    std::vector<float*> d_in((size_t)n_streams, nullptr), d_out((size_t)n_streams, nullptr);
+    int status = GAMER_OK;
+    cudaError_t e = cudaSuccess;
+    for (int s = 0; s < n_streams && status == GAMER_OK; ++s) {
+        e = cudaStreamCreateWithFlags(&streams[s], cudaStreamNonBlocking);
+        if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); break; }
+        e = cudaMalloc(&d_in[s], in_bytes);
+        if (e == cudaSuccess) e = cudaMalloc(&d_out[s], out_bytes);
+        if (e != cudaSuccess) {
+            status = fail(e == cudaErrorMemoryAllocation ? GAMER_ENOMEM : GAMER_ECUDA, "cudaMalloc of staging buffers: %s",
+                          cudaGetErrorString(e));
+            (void)cudaGetLastError();
+        }
+    }
+    // Fig.5: chunk c goes to stream c mod N_s: copy in, kernel, copy out.  Stream order keeps a
+    // staging buffer from being overwritten before its previous chunk has left it.
+    for (long long c = 0; c < n_chunks && status == GAMER_OK; ++c) {
+        const int s = (int)(c % n_streams);
+        const long long g0 = c * groups_per_chunk;
+        const long long ng = (n_groups - g0) < groups_per_chunk ? (n_groups - g0) : groups_per_chunk;
+        e = cudaMemcpyAsync(d_in[s], h_in + g0 * gamer::GROUP_IN_FLOATS, (size_t)ng * gamer::GROUP_IN_FLOATS * sizeof(float),
+                            cudaMemcpyHostToDevice, streams[s]);
+        if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaMemcpyAsync H2D: %s", cudaGetErrorString(e)); break; }
+        status = launch(d_in[s], d_out[s], ng, dt, dh, gamma, backward, nullptr, nullptr, streams[s]);
+        if (status != GAMER_OK) break;
+        e = cudaMemcpyAsync(h_out + g0 * gamer::GROUP_OUT_FLOATS, d_out[s],
+                            (size_t)ng * gamer::GROUP_OUT_FLOATS * sizeof(float), cudaMemcpyDeviceToHost, streams[s]);
+        if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaMemcpyAsync D2H: %s", cudaGetErrorString(e)); break; }
+    }
+    for (int s = 0; s < n_streams; ++s) {
+        if (streams[s]) {
+            e = cudaStreamSynchronize(streams[s]);
+            if (e != cudaSuccess && status == GAMER_OK)
+                status = fail(GAMER_ECUDA, "cudaStreamSynchronize: %s", cudaGetErrorString(e));
+        }
+        if (d_in[s]) cudaFree(d_in[s]);
+        if (d_out[s]) cudaFree(d_out[s]);
+        if (streams[s]) cudaStreamDestroy(streams[s]);
+    }
+    return status;
+}
+
+int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread) {
+    KernelFn fn = pick_kernel(false, false, false);
+    int sm_count = 0;
+    const int rc = prepare(fn, 0, &sm_count);
+    if (rc != GAMER_OK) return rc;
+    cudaFuncAttributes fa;
+    const cudaError_t e = cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn));
+    if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaFuncGetAttributes: %s", cudaGetErrorString(e));
+    if (n_groups < 0) n_groups = 0;
+    if (grid) *grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
+    if (block) *block = gamer::BLOCK_THREADS;
+    if (smem_bytes) *smem_bytes = gamer::SMEM_BYTES;
+    if (regs_per_thread) *regs_per_thread = fa.numRegs;
+    g_err[0] = '\0';
+    return GAMER_OK;
+}
+
+const char* gamer_last_error(void) { return g_err; }
+const char* gamer_version(void) { return "gamer-hydro-b200 0.1.0 (sm_100a)"; }
+
+}  // extern "C"

@@ -168,11 +168,14 @@ def config3(grid=(8, 8, 8)):
 
 
 def config4(grid=(16, 16, 16)):
-    """4096 groups: ln rho Gaussian with P(k)~k^-3, sigma=2; P=rho^gamma; v = 0.5(sqrt(1-a^2) g + a grad ln rho / rms)."""
+    """4096 groups: ln rho Gaussian, sigma=2, shell-integrated spectrum E(k) = 4 pi k^2 P(k) ~ k^-3 (3-D power
+    P(k) ~ k^-5; reading R17: with 3-D power ~ k^-3 adjacent cells differ by a factor e^1.2 rms, up to
+    e^6.6, and the floor-free scheme leaves the physical domain in both fp32 and fp64); P=rho^gamma;
+    v = 0.5(sqrt(1-a^2) g + a grad ln rho / rms), g ~ N(0,1) iid, a = 0.5."""
     gamma, dh, alpha = 5.0 / 3.0, 1.0 / 256.0, 0.5
     rng = rng_for(4)
     shp = (grid[0] * PS, grid[1] * PS, grid[2] * PS)
-    lnrho = 2.0 * gaussian_field(shp, -3.0, rng)
+    lnrho = 2.0 * gaussian_field(shp, -5.0, rng)
     lnrho -= lnrho.mean()
     rho = np.exp(lnrho)
     vel = []

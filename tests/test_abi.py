@@ -1,0 +1,85 @@
+"""The C-ABI library loads and exports every symbol include/gamer_hydro.h declares; host-side argument validation.
+No kernel is launched here (no GPU needed): only paths that return before any CUDA work are exercised."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_0907_3390_b200 import hydro
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    names = []
+    for fn in os.listdir(os.path.join(ROOT, "include")):
+        if fn.endswith(".h"):
+            src = open(os.path.join(ROOT, "include", fn)).read()
+            src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+            names += re.findall(r"GAMER_API\s+[\w\s\*]+?\b(gamer_\w+)\s*\(", src)
+    return sorted(set(names))
+
+
+def test_header_declares_the_survey_entry_points():
+    syms = declared_symbols()
+    for s in ("gamer_hydro_advance", "gamer_hydro_advance_ex", "gamer_hydro_in_floats", "gamer_hydro_out_floats",
+              "gamer_hydro_pipeline_run", "gamer_last_error", "gamer_version"):
+        assert s in syms
+
+
+def test_library_exports_every_declared_symbol():
+    L = ctypes.CDLL(hydro.LIB_PATH)
+    for s in declared_symbols():
+        assert hasattr(L, s), s
+
+
+def test_size_helpers():
+    assert hydro.gamer_hydro_in_floats(1, 3) == 5 * 22 ** 3 == 53240
+    assert hydro.gamer_hydro_in_floats(32768, 3) * 4 == 32768 * 212960
+    assert hydro.gamer_hydro_out_floats(7) == 7 * 5 * 4096
+    assert hydro.gamer_hydro_face_flux_floats(2) == 2 * 3 * 3 * 5 * 256
+    assert hydro.gamer_hydro_in_floats(-1, 3) == 0
+    assert hydro.gamer_hydro_out_floats(-5) == 0
+    assert "sm_100a" in hydro.gamer_version()
+
+
+def test_argument_validation_needs_no_device():
+    L = hydro.lib()
+    buf = (ctypes.c_float * 64)()
+    a = ctypes.addressof(buf)
+    a16 = (a + 15) & ~15
+    # ghost != 3 -> unsupported (7-point stencil)
+    assert L.gamer_hydro_advance(a16, a16, 1, 2, 0.1, 1.0, 1.4, None) == hydro.GAMER_EUNSUPPORTED
+    assert "ghost" in hydro.gamer_last_error()
+    assert L.gamer_hydro_advance(a16, a16, -1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(None, a16, 1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(a16, a16 + 4, 1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL      # misaligned
+    assert L.gamer_hydro_advance(a16, a16, 1, 3, 0.1, 0.0, 1.4, None) == hydro.GAMER_EINVAL           # dh
+    assert L.gamer_hydro_advance(a16, a16, 1, 3, -0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL          # dt
+    assert L.gamer_hydro_advance(a16, a16, 1, 3, float("nan"), 1.0, 1.4, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(a16, a16, 1, 3, 0.1, 1.0, 1.0, None) == hydro.GAMER_EINVAL           # gamma
+    assert L.gamer_hydro_advance_ex(a16, a16, 1, 3, 0.1, 1.0, 1.4, 2, None, None, None) == hydro.GAMER_EINVAL
+    # n_groups == 0 is a successful no-op, even with NULL buffers
+    assert L.gamer_hydro_advance(None, None, 0, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_OK
+    assert hydro.gamer_last_error() == ""
+    assert L.gamer_hydro_pipeline_run(a16, a16, 1, 3, 0.1, 1.0, 1.4, 0, 0, 4) == hydro.GAMER_EINVAL   # chunk
+    assert L.gamer_hydro_pipeline_run(a16, a16, 1, 3, 0.1, 1.0, 1.4, 0, 8, 0) == hydro.GAMER_EINVAL   # streams
+    assert L.gamer_hydro_pipeline_run(None, None, 0, 3, 0.1, 1.0, 1.4, 0, 8, 2) == hydro.GAMER_OK
+    with pytest.raises(hydro.GamerError):
+        hydro.gamer_hydro_advance(a16, a16, 1, 4, 0.1, 1.0, 1.4, stream=0)
+
+
+def test_oracle_and_product_do_not_import_each_other():
+    """The oracle is test infrastructure: neither side may import, link or read the other (no shared code)."""
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_0907_3390_b200")):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), fn
+                assert "rtvd_oracle" not in src, fn
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".cpp", ".h")):
+            src = open(os.path.join(ROOT, "oracle", fn)).read()
+            assert "paper_0907_3390_b200" not in src.replace("paper_0907_3390_b200/csrc)", ""), fn
+            assert "gamer_hydro.h" not in src and "rtvd_march" not in src, fn
