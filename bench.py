@@ -263,7 +263,7 @@ def run_ours(args):
 
     # end to end through the public C-ABI call with host buffers
     e2e = None
-    if rank == 0 or world > 1:
+    if (rank == 0 or world > 1) and not args.no_e2e:
         try:
             h_in = torch.empty(d_in.shape, dtype=torch.float32, pin_memory=True)
             h_out = torch.empty(d_out.shape, dtype=torch.float32, pin_memory=True)
@@ -323,6 +323,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=2048, help="pipeline: groups per chunk (N_g)")
     ap.add_argument("--streams", type=int, default=4, help="pipeline: number of streams (N_s)")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
     ap.add_argument("--no-check", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

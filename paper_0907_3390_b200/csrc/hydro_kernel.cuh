@@ -12,13 +12,21 @@
 
 namespace gamer {
 
-constexpr int BLOCK_THREADS = 512;
+#ifndef GAMER_BLOCK_THREADS
+#define GAMER_BLOCK_THREADS 512
+#endif
+constexpr int BLOCK_THREADS = GAMER_BLOCK_THREADS;
 constexpr int GROUP_IN_FLOATS = NCOMP * NP * NP * NP;     // 53 240
 constexpr int GROUP_OUT_FLOATS = NCOMP * PS * PS * PS;    // 20 480
 constexpr int GROUP_FACE_FLOATS = 3 * 3 * NCOMP * PS * PS;
 constexpr int GROUP_IN_BYTES = GROUP_IN_FLOATS * 4;       // 212 960
 constexpr int VAR_FLOATS = NP * NP * NP;                  // 10 648
 constexpr int SMEM_BYTES = GROUP_IN_BYTES + 64;           // + mbarrier and reduction scratch
+
+#ifdef GAMER_PHASE_TIMERS
+// debug builds only (never defined by build.py): per-CTA cycles spent waiting for the load / in each sweep
+__device__ long long g_phase_cycles[1024 * 4];
+#endif
 
 // ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -54,14 +62,39 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 
 // ---- sinks ------------------------------------------------------------------------------------------------------
 // Writes the updated cells back into the row in shared memory (in place); optionally the face fluxes to HBM.
+// Along x (STRIDE 1) an even cell is held back one step and stored together with its odd right neighbour as one
+// 64-bit store (cells 3 and 18 have no partner and go out alone).
 template <int STRIDE>
 struct SmemSink {
     float* dst[NCOMP];       // row-local component order, cell 0 of the row
     float* fptr[NCOMP];      // &face_flux[g][d][0][var(q)][b][a], or unused
     bool face_row;
+    float held[NCOMP];
+    template <int ODD>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
+        if (STRIDE == 1) {
+            if (ODD) {
+                if (j == NG) {
 #pragma unroll
-        for (int k = 0; k < NCOMP; ++k) dst[k][j * STRIDE] = u[k];
+                    for (int k = 0; k < NCOMP; ++k) dst[k][j] = u[k];
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k)
+                        *reinterpret_cast<float2*>(dst[k] + j - 1) = make_float2(held[k], u[k]);
+                }
+            } else {
+                if (j == NG + PS - 1) {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) dst[k][j] = u[k];
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) held[k] = u[k];
+                }
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) dst[k][j * STRIDE] = u[k];
+        }
     }
     __device__ __forceinline__ void face(int p, const float (&f)[NCOMP]) {
         if (face_row) {
@@ -80,13 +113,34 @@ struct FinalSink {
     bool face_row;
     float gm1, ggm1;
     float speed;             // running max of c_s + max|v_i|
+    float held[NCOMP];
+    template <int ODD>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
+        if (TO_GLOBAL) {
 #pragma unroll
-        for (int k = 0; k < NCOMP; ++k) {
-            if (TO_GLOBAL)
-                dst[k][(j - NG) * OSTRIDE] = u[k];
-            else
-                dst[k][j * STRIDE] = u[k];
+            for (int k = 0; k < NCOMP; ++k) dst[k][(j - NG) * OSTRIDE] = u[k];
+        } else if (STRIDE == 1) {
+            if (ODD) {
+                if (j == NG) {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) dst[k][j] = u[k];
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k)
+                        *reinterpret_cast<float2*>(dst[k] + j - 1) = make_float2(held[k], u[k]);
+                }
+            } else {
+                if (j == NG + PS - 1) {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) dst[k][j] = u[k];
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) held[k] = u[k];
+                }
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) dst[k][j * STRIDE] = u[k];
         }
         if (WANT_SPEED) {    // Eq.30 on the updated cell
             const float rinv = 1.0f / u[0];
@@ -125,9 +179,27 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
     constexpr int OSTRIDE = D == 0 ? 1 : (D == 1 ? PS : PS * PS);
     constexpr int OSTR_A = AX_A == 0 ? 1 : PS;
     constexpr int OSTR_B = AX_B == 1 ? PS : PS * PS;
+#ifdef GAMER_DUP_ROWS      // timing experiment only: surplus threads redo rows (results are garbage)
+    const int t = threadIdx.x % (N_A * N_B);
+#else
     const int t = threadIdx.x;
     if (t >= N_A * N_B) return;
-    const int a = LO_A + t % N_A, b = LO_B + t / N_A;         // padded transverse coordinates
+#endif
+    // padded transverse coordinates of this thread's row.  Where the fast axis is the 16 interior x cells, the two
+    // half-warps are placed 16 banks apart (y sweep: z and z+4; z sweep: y and y+8) so that the 4-byte accesses of a
+    // warp hit 32 different banks; rows along x are 8-byte accessed and conflict-free for consecutive rows.
+    int a, b;
+    if (D == 1 && N_A == PS && N_B == NP) {
+        const int w = t >> 5, h = (t >> 4) & 1;
+        a = LO_A + (t & 15);
+        b = w < 10 ? 8 * (w >> 2) + (w & 3) + 4 * h : 18 + h;
+    } else if (D == 2 && N_A == PS && N_B == PS) {
+        a = LO_A + (t & 15);
+        b = LO_B + (t >> 5) + 8 * ((t >> 4) & 1);
+    } else {
+        a = LO_A + t % N_A;
+        b = LO_B + t / N_A;
+    }
     const int base = a * STR_A + b * STR_B;
     const float* src[NCOMP];
 #pragma unroll
@@ -178,8 +250,17 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
     }
     __syncthreads();
 
+#ifdef GAMER_PHASE_TIMERS
+    long long tacc[5] = {0, 0, 0, 0, 0}, tt0, tt1;
+#define PHASE_T0() tt0 = clock64()
+#define PHASE_ACC(i) do { tt1 = clock64(); tacc[i] += tt1 - tt0; tt0 = tt1; } while (0)
+#else
+#define PHASE_T0()
+#define PHASE_ACC(i)
+#endif
     uint32_t parity = 0;
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
+        PHASE_T0();
         if (threadIdx.x == 0) {
             fence_proxy_async();      // generic-proxy accesses of the previous group are ordered before the async write
             mbar_expect_tx(bar, GROUP_IN_BYTES);
@@ -189,6 +270,7 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
         }
         mbar_wait(bar, parity);
         parity ^= 1u;
+        PHASE_ACC(0);
 
         float* out_g = out + g * (long long)GROUP_OUT_FLOATS;
         float* face_g = WANT_FACE ? face_flux + g * (long long)GROUP_FACE_FLOATS : nullptr;
@@ -196,8 +278,10 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
         if (!BACKWARD) {
             sweep<0, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);   // x: (y,z) all
             __syncthreads();
+            PHASE_ACC(1);
             sweep<1, NG, PS, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);  // y: x int, z all
             __syncthreads();
+            PHASE_ACC(2);
             sweep<2, NG, PS, NG, PS, true, true, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed);   // z
         } else {
             sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);   // z: (x,y) all
@@ -227,7 +311,12 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             }
         }
         __syncthreads();     // every thread is done with the buffer before the next bulk copy overwrites it
+        PHASE_ACC(3);
     }
+#ifdef GAMER_PHASE_TIMERS
+    if (threadIdx.x == 0)
+        for (int i = 0; i < 4; ++i) g_phase_cycles[blockIdx.x * 4 + i] = tacc[i];
+#endif
 }
 
 }  // namespace gamer

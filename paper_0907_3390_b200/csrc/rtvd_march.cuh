@@ -20,8 +20,13 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#ifndef GAMER_MARCH_UNROLL
+#define GAMER_MARCH_UNROLL 2     /* pairs of cells per loop body */
+#endif
+
 namespace gamer {
 
+constexpr int MARCH_UNROLL = GAMER_MARCH_UNROLL;
 constexpr int NCOMP = 5;
 constexpr int PS = 16;
 constexpr int NG = 3;
@@ -47,6 +52,8 @@ __device__ __forceinline__ float sqrt_fast(float x) {
 
 // Cell-centred G^R = c u + F and G^L = c u - F of one cell; u = (rho, m_n, m_t1, m_t2, e), m_n normal to the sweep.
 // c = |v_n| + c_s (reading R1), P from all three momenta (Eqs.4-5, reading R2).
+// (Blackwell's packed FFMA2/FADD2/FMUL2 were tried for the 5-vector operations: fewer instructions, no gain — a packed
+// instruction holds the issue port for two cycles on this part.)
 __device__ __forceinline__ void cell_split_flux(const float (&u)[NCOMP], const GasConst& gc, float (&gr)[NCOMP],
                                                 float (&gl)[NCOMP]) {
     const float rinv = rcp_fast(u[0]);
@@ -73,6 +80,7 @@ __device__ __forceinline__ void cell_split_flux(const float (&u)[NCOMP], const G
 }
 
 // base + a b / (a + b) if a b > 0, else base     (sgn = +1)   |   base - a b / (a + b) ...   (sgn = -1)
+// A select on the sign of the product, never a mask (reading R6).
 template <int SGN>
 __device__ __forceinline__ float limited(float base, float a, float b) {
     const float p = a * b;
@@ -83,45 +91,47 @@ __device__ __forceinline__ float limited(float base, float a, float b) {
 
 // Marches one row.  `src[q]` points to cell 0 of component q (row-local order), element n at src[q][n * STRIDE].
 // Sink must provide:
-//   void cell(int j, const float (&u)[5])   updated cell j = 3..18, row-local component order
+//   template <int ODD> void cell(int j, const float (&u)[5])   updated cell j = 3..18 (ODD = j & 1, static),
+//                                            row-local component order
 //   void face(int p, const float (&f)[5])   true flux F^{t+dt/2} through interface 2|3 (p=0), 10|11 (1), 18|19 (2);
 //                                            called only if WANT_FACE
-// The original value of cell j is re-read from src just before cell(j) is called, so a Sink may overwrite the row in
-// place at index j (and only there).
+// A Sink may overwrite the row in place at index j (the march never reads cell j again).
+//
+// The march is a software pipeline of depth 6: at step n it loads cell n, forms the first-order flux through (n-1|n),
+// the midpoint state of cell m = n-1, the limited fluxes through (m-2|m-1) and the new value of cell m-2 = n-3.
+// Steps 0..5 fill the pipeline (PH = n, statically pruned); steps 6..21 are identical and run as a rolled loop
+// (PH = 6) so that the code of all three sweeps stays resident in the instruction cache.
 template <int STRIDE, bool WANT_FACE, class Sink>
-__device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], const GasConst& gc, Sink& sink) {
-    float u_prev[NCOMP];                       // u_{n-1}
+struct RowMarch {
+    float u1[NCOMP], u2[NCOMP], u3[NCOMP];     // u_{n-1}, u_{n-2}, u_{n-3} (the originals, kept for Eqs.13-14)
     float gr1_prev[NCOMP];                     // G^R_{n-1} at time t
-    float f_prev[NCOMP];                       // 2F_{n-3/2}
+    float f_prev[NCOMP];                       // 2F through (n-2|n-1)
     float gr2_prev[NCOMP], gl2_prev[NCOMP];    // midpoint G^R, G^L of cell m-1
     float gr2_pp[NCOMP];                       // midpoint G^R of cell m-2
     float ar1[NCOMP], ar2[NCOMP], al1[NCOMP];  // ar1 = G^R_{m-1}-G^R_{m-2}, ar2 = G^R_{m-2}-G^R_{m-3}, al1 likewise for L
     float fh_prev[NCOMP];                      // 2F^h through the previous limited interface
 
-#pragma unroll
-    for (int n = 0; n < NP; ++n) {
-        float u[NCOMP], gr1[NCOMP], gl1[NCOMP];
-#pragma unroll
-        for (int k = 0; k < NCOMP; ++k) u[k] = src[k][n * STRIDE];
+    template <int PH>
+    __device__ __forceinline__ void step(const float (&u)[NCOMP], int n, const GasConst& gc, Sink& sink) {
+        float gr1[NCOMP], gl1[NCOMP];
         cell_split_flux(u, gc, gr1, gl1);                                   // (a)
-        if (n >= 1) {
+        if (PH >= 1) {
             float f[NCOMP];
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) f[k] = gr1_prev[k] - gl1[k];     // (b) interface (n-1 | n)
-            if (n >= 2) {
-                const int m = n - 1;                                        // midpoint cell
+            if (PH >= 2) {                                                  // midpoint cell m = n-1
                 float uh[NCOMP], gr2[NCOMP], gl2[NCOMP];
 #pragma unroll
-                for (int k = 0; k < NCOMP; ++k) uh[k] = fmaf(-gc.kq, f[k] - f_prev[k], u_prev[k]);   // (c)
+                for (int k = 0; k < NCOMP; ++k) uh[k] = fmaf(-gc.kq, f[k] - f_prev[k], u1[k]);   // (c)
                 cell_split_flux(uh, gc, gr2, gl2);                          // (d)
-                if (m >= 2) {
+                if (PH >= 3) {                                              // m >= 2
                     float ar0[NCOMP], al0[NCOMP];
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) {
                         ar0[k] = gr2[k] - gr2_prev[k];                      // G^R_m - G^R_{m-1}
                         al0[k] = gl2[k] - gl2_prev[k];                      // G^L_m - G^L_{m-1}
                     }
-                    if (m >= 4) {                                           // (e) interface (m-2 | m-1)
+                    if (PH >= 5) {                                          // m >= 4: (e) interface (m-2 | m-1)
                         float fh[NCOMP];
 #pragma unroll
                         for (int k = 0; k < NCOMP; ++k) {
@@ -131,7 +141,7 @@ __device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], con
                             fh[k] = xr - xl;
                         }
                         if (WANT_FACE) {
-                            const int i = m - 2;                            // interface (i | i+1)
+                            const int i = n - 3;                            // interface (i | i+1), i = m-2
                             if (i == NG - 1 || i == NG + PS / 2 - 1 || i == NG + PS - 1) {
                                 float ff[NCOMP];
 #pragma unroll
@@ -139,13 +149,11 @@ __device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], con
                                 sink.face(i == NG - 1 ? 0 : (i == NG + PS - 1 ? 2 : 1), ff);
                             }
                         }
-                        if (m >= 5) {                                       // (f) cell j = m-2
-                            const int j = m - 2;
+                        if (PH >= 6) {                                      // m >= 5: (f) cell j = m-2 = n-3
                             float un[NCOMP];
 #pragma unroll
-                            for (int k = 0; k < NCOMP; ++k)
-                                un[k] = fmaf(-gc.kh, fh[k] - fh_prev[k], src[k][j * STRIDE]);
-                            sink.cell(j, un);
+                            for (int k = 0; k < NCOMP; ++k) un[k] = fmaf(-gc.kh, fh[k] - fh_prev[k], u3[k]);
+                            sink.template cell<(PH + 1) & 1>(n - 3, un);      // parity of j = n-3 is static
                         }
 #pragma unroll
                         for (int k = 0; k < NCOMP; ++k) fh_prev[k] = fh[k];
@@ -169,10 +177,48 @@ __device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], con
         }
 #pragma unroll
         for (int k = 0; k < NCOMP; ++k) {
-            u_prev[k] = u[k];
+            if (PH >= 2) u3[k] = u2[k];
+            if (PH >= 1) u2[k] = u1[k];
+            u1[k] = u[k];
             gr1_prev[k] = gr1[k];
         }
     }
+
+    // Cells are fetched two at a time (n even, n+1): a row along x is read with 64-bit shared-memory loads.
+    template <int PH0, int PH1>
+    __device__ __forceinline__ void pair(const float* const (&src)[NCOMP], int n, const GasConst& gc, Sink& sink) {
+        float ua[NCOMP], ub[NCOMP];
+        if (STRIDE == 1) {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                const float2 t = *reinterpret_cast<const float2*>(src[k] + n);
+                ua[k] = t.x;
+                ub[k] = t.y;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                ua[k] = src[k][n * STRIDE];
+                ub[k] = src[k][(n + 1) * STRIDE];
+            }
+        }
+        step<PH0>(ua, n, gc, sink);
+        step<PH1>(ub, n + 1, gc, sink);
+    }
+
+    __device__ __forceinline__ void run(const float* const (&src)[NCOMP], const GasConst& gc, Sink& sink) {
+        pair<0, 1>(src, 0, gc, sink);
+        pair<2, 3>(src, 2, gc, sink);
+        pair<4, 5>(src, 4, gc, sink);
+#pragma unroll MARCH_UNROLL
+        for (int n = 6; n < NP; n += 2) pair<6, 6>(src, n, gc, sink);
+    }
+};
+
+template <int STRIDE, bool WANT_FACE, class Sink>
+__device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], const GasConst& gc, Sink& sink) {
+    RowMarch<STRIDE, WANT_FACE, Sink> m;
+    m.run(src, gc, sink);
 }
 
 }  // namespace gamer
