@@ -97,6 +97,37 @@ class ClockSampler(threading.Thread):
                     samples=len(self.samples))
 
 
+def profiled_traffic(config, n_groups):
+    """DRAM bytes per launch of the hydro kernel from the committed ncu capture (profiles/), if it matches the workload."""
+    import csv
+    best = None
+    pdir = os.path.join(ROOT, "profiles")
+    if not os.path.isdir(pdir):
+        return None
+    for fn in sorted(os.listdir(pdir)):
+        if fn.endswith("_traffic.csv"):
+            with open(os.path.join(pdir, fn)) as f:
+                for row in csv.DictReader(f):
+                    if row["workload"] == "config%d" % config and int(row["n_groups"]) == n_groups:
+                        best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    return best
+
+
+def max_over_ranks(x, dist, device):
+    """max of a python float over all ranks (identity without a process group); device = where the tensor lives."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(world, units_per_rank, seconds_max):
+    """whole-job metric for independent replicas: all ranks' units over the slowest rank's time."""
+    return world * units_per_rank / seconds_max
+
+
 def physical_gpu_index(local):
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -226,12 +257,9 @@ def run_ours(args):
         dist.barrier()
     total_ms = evs[0].elapsed_time(evs[-1])
     per_launch_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
-    if dist is not None:
-        t = torch.tensor([total_ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, device)
     ms_per_step = total_ms / args.steps
-    value = world * n * CELLS_PER_GROUP / (ms_per_step * 1e-3)
+    value = job_throughput(world, n * CELLS_PER_GROUP, ms_per_step * 1e-3)
     kernel_ms = float(np.mean(per_launch_ms))
 
     # spot check of the timed output against the oracle (a few groups), so that a wrong-but-fast run cannot pass
@@ -258,6 +286,11 @@ def run_ours(args):
     t_alu = FLOPS_PER_GROUP / (fp32_peak_tflops * 1e12)
     t_hbm = BYTES_PER_GROUP / (peaks["hbm_gbs"] * 1e9)
     roofline = dict(roofline_alu if t_alu >= t_hbm else roofline_hbm)
+    traffic = profiled_traffic(args.config, n)
+    for r in (roofline, roofline_hbm, roofline_alu):
+        r["traffic"] = traffic
+    roofline["algorithmic_bytes"] = n * BYTES_PER_GROUP
+    roofline["algorithmic_flops"] = n * FLOPS_PER_GROUP
     roofline["kernel_ms"] = kernel_ms
     roofline["ns_per_group"] = kernel_ms * 1e6 / n
 
@@ -278,11 +311,8 @@ def run_ours(args):
             for _ in range(e2e_steps):
                 hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, dt, dh, gamma, 0, chunk, ns)
             wall = time.perf_counter() - t0
-            if dist is not None:
-                t = torch.tensor([wall], device=device, dtype=torch.float64)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                wall = float(t.item())
-            e2e = dict(value=world * e2e_steps * n * CELLS_PER_GROUP / wall, unit=UNIT,
+            wall = max_over_ranks(wall, dist, device)
+            e2e = dict(value=job_throughput(world, e2e_steps * n * CELLS_PER_GROUP, wall), unit=UNIT,
                        h2d_bytes_per_step=int(h_in.numel() * 4), d2h_bytes_per_step=int(h_out.numel() * 4),
                        steps=e2e_steps, ms_per_step=1e3 * wall / e2e_steps, groups_per_chunk=chunk, n_streams=ns,
                        h2d_gbs=h_in.numel() * 4 * e2e_steps / wall / 1e9, api="gamer_hydro_pipeline_run (pinned host)")
