@@ -8,7 +8,11 @@
 //       64-byte segments; backward: in place, then a 128-bit coalesced copy-out)
 #pragma once
 #include <cstdint>
+#ifdef GAMER_PACKED
+#include "rtvd_march_pk.cuh"
+#else
 #include "rtvd_march.cuh"
+#endif
 
 namespace gamer {
 

@@ -57,15 +57,16 @@ __device__ __forceinline__ float sqrt_fast(float x) {
 __device__ __forceinline__ void cell_split_flux(const float (&u)[NCOMP], const GasConst& gc, float (&gr)[NCOMP],
                                                 float (&gl)[NCOMP]) {
     const float rinv = rcp_fast(u[0]);
-    const float v = u[1] * rinv;
-    float q = u[2] * u[2];
+    const float v = __fmul_rn(u[1], rinv);
+    float q = __fmul_rn(u[2], u[2]);
     q = fmaf(u[3], u[3], q);
     q = fmaf(u[1], u[1], q);
-    const float hk = 0.5f * rinv;
+    const float hk = __fmul_rn(0.5f, rinv);
     const float eint = fmaf(-q, hk, u[4]);          // e - rho v^2 / 2
-    const float P = gc.gm1 * eint;
-    const float cs = sqrt_fast((gc.ggm1 * eint) * rinv);
-    const float c = fabsf(v) + cs;
+    const float P = __fmul_rn(gc.gm1, eint);
+    const float cs = sqrt_fast(__fmul_rn(__fmul_rn(gc.ggm1, eint), rinv));
+    const float c = __fadd_rn(fabsf(v), cs);
+#ifdef GAMER_SPLIT_CUF
     float F[NCOMP];
     F[0] = u[1];
     F[1] = fmaf(u[1], v, P);
@@ -77,6 +78,25 @@ __device__ __forceinline__ void cell_split_flux(const float (&u)[NCOMP], const G
         gr[k] = fmaf(c, u[k], F[k]);
         gl[k] = fmaf(c, u[k], -F[k]);
     }
+#else
+    // G^R = c u + F = u (c + v) + (0, P, 0, 0, P v),  G^L = c u - F = u (c - v) - (0, P, 0, 0, P v):  F = u v + (0, P, 0, 0, P v).
+    // Two instructions fewer per cell than c u +- F, and every multiply shares the operand c +- v with its neighbours
+    // (operand-reuse cache: the register file delivers two operands per clock, a 3-register FFMA takes 1.5).
+    // Explicit intrinsics: no FMA contraction, so every cell is computed by the same operations wherever it sits in the
+    // pipeline (a uniform state must come back bit-exactly).
+    const float cp = __fadd_rn(c, v), cm = __fsub_rn(c, v);
+    const float Pv = __fmul_rn(P, v);
+    gr[0] = __fmul_rn(u[0], cp);
+    gr[1] = fmaf(u[1], cp, P);
+    gr[2] = __fmul_rn(u[2], cp);
+    gr[3] = __fmul_rn(u[3], cp);
+    gr[4] = fmaf(u[4], cp, Pv);
+    gl[0] = __fmul_rn(u[0], cm);
+    gl[1] = fmaf(u[1], cm, -P);
+    gl[2] = __fmul_rn(u[2], cm);
+    gl[3] = __fmul_rn(u[3], cm);
+    gl[4] = fmaf(u[4], cm, -Pv);
+#endif
 }
 
 // base + a b / (a + b) if a b > 0, else base     (sgn = +1)   |   base - a b / (a + b) ...   (sgn = -1)
