@@ -1,6 +1,7 @@
 // gamer_hydro.cu — the C ABI of include/gamer_hydro.h: argument validation, launch, and the stream pipeline.
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
@@ -104,6 +105,8 @@ gamer::GasConst make_const(float dt, float dh, float gamma) {
     gc.ggm1 = gamma * (gamma - 1.0f);
     gc.kq = 0.25f * k;
     gc.kh = 0.5f * k;
+    gc.kq_gm1 = gc.kq * gc.gm1;
+    gc.kq_sg = gc.kq * sqrtf(gc.ggm1);
     return gc;
 }
 

@@ -8,10 +8,10 @@
 //       64-byte segments; backward: in place, then a 128-bit coalesced copy-out)
 #pragma once
 #include <cstdint>
-#ifdef GAMER_PACKED
-#include "rtvd_march_pk.cuh"
-#else
+#ifdef GAMER_MARCH_V1
 #include "rtvd_march.cuh"
+#else
+#include "rtvd_march2.cuh"
 #endif
 
 namespace gamer {

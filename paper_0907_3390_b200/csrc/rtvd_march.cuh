@@ -37,6 +37,8 @@ struct GasConst {
     float ggm1;   // gamma (gamma - 1)
     float kq;     // (dt/dh) / 4
     float kh;     // (dt/dh) / 2
+    float kq_gm1;   // kq (gamma - 1)
+    float kq_sg;    // kq sqrt(gamma (gamma - 1))
 };
 
 __device__ __forceinline__ float rcp_fast(float x) {

@@ -1,0 +1,258 @@
+// rtvd_march2.cuh — the 1-D relaxing-TVD row update as a register sliding window (device code, sm_100a), version 2.
+//
+// One thread owns one row of 22 cells along the sweep direction and marches along it once (see rtvd_march.cuh for the
+// first version; the arithmetic of Eqs.9-14 is unchanged).  What is different here is only how much is computed and
+// carried per cell:
+//
+//  * half step (Eqs.8 and 13, :138, :168).  With G^R = c u + F = u (c + v) + Pi, G^L = c u - F = u (c - v) - Pi,
+//    Pi = (0, P, 0, 0, P v), and q = (dt/dh)/4, substituting the first-order fluxes 2F_{n+1/2} = G^R_n - G^L_{n+1} into
+//    Eq.13 gives
+//        u^h_n = u_n - q (G^R_n + G^L_n) + q G^L_{n+1} + q G^R_{n-1}
+//              = (1 - 2 q c_n) u_n  +  q (c - v)_{n+1} u_{n+1}  +  q (c + v)_{n-1} u_{n-1}  +  q (Pi_{n-1} - Pi_{n+1}).
+//    So the time-t split fluxes are never formed: each cell contributes three scalars (q(c+v), q(c-v), 1-2qc) and
+//    the two non-zero entries of q Pi, and a midpoint component costs 3 FMA-pipe instructions (4 for m_n and e).
+//  * limited fluxes (Eqs.9-12).  The right-moving flux through (m-1|m) only needs cells m-2..m, so it is formed one
+//    step ahead of the left-moving flux through the same interface and carried; every window is then one or two deep.
+//
+// Every cell is computed by the same instruction sequence wherever it sits in the row, so a uniform state (and a
+// transverse sweep of 1-D data) comes back bit-exactly: equal midpoint states give equal fluxes and Eq.14 subtracts 0.
+#pragma once
+#include <cuda_runtime.h>
+
+#ifndef GAMER_MARCH_UNROLL
+#define GAMER_MARCH_UNROLL 2     /* pairs of cells per loop body */
+#endif
+
+namespace gamer {
+
+constexpr int MARCH_UNROLL = GAMER_MARCH_UNROLL;
+constexpr int NCOMP = 5;
+constexpr int PS = 16;
+constexpr int NG = 3;
+constexpr int NP = PS + 2 * NG;   // 22
+
+struct GasConst {
+    float gm1;      // gamma - 1
+    float ggm1;     // gamma (gamma - 1)
+    float kq;       // (dt/dh) / 4
+    float kh;       // (dt/dh) / 2
+    float kq_gm1;   // kq (gamma - 1)
+    float kq_sg;    // kq sqrt(gamma (gamma - 1))
+};
+
+__device__ __forceinline__ float rcp_fast(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float sqrt_fast(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// What a cell at time t contributes to the half step of its neighbours and of itself (all times q = (dt/dh)/4).
+struct HalfCoef {
+    float cp;     // q (c + v)
+    float cm;     // q (c - v)
+    float sig;    // 1 - 2 q c
+    float P;      // q P
+    float Pv;     // q P v
+};
+
+// u = (rho, m_n, m_t1, m_t2, e), m_n normal to the sweep.  c = |v_n| + c_s (reading R1), P from all three
+// momenta (Eqs.4-5, reading R2).
+__device__ __forceinline__ HalfCoef half_coef(const float (&u)[NCOMP], const GasConst& gc) {
+    HalfCoef h;
+    const float rinv = rcp_fast(u[0]);
+    const float v = __fmul_rn(u[1], rinv);
+    float q = __fmul_rn(u[2], u[2]);
+    q = fmaf(u[3], u[3], q);
+    q = fmaf(u[1], u[1], q);
+    const float hk = __fmul_rn(0.5f, rinv);
+    const float eint = fmaf(-q, hk, u[4]);                          // e - rho v^2 / 2
+    h.P = __fmul_rn(gc.kq_gm1, eint);
+    const float s = sqrt_fast(__fmul_rn(eint, rinv));
+    const float vq = __fmul_rn(gc.kq, v);
+    const float c = __fadd_rn(fabsf(vq), __fmul_rn(gc.kq_sg, s));   // q (|v| + c_s)
+    h.cp = __fadd_rn(c, vq);
+    h.cm = __fsub_rn(c, vq);
+    h.sig = fmaf(-2.0f, c, 1.0f);
+    h.Pv = __fmul_rn(h.P, v);
+    return h;
+}
+
+// Cell-centred G^R = c u + F = u (c + v) + (0, P, 0, 0, P v) and G^L = c u - F = u (c - v) - (0, P, 0, 0, P v) of the
+// midpoint state (2 F^R and 2 F^L of Eq.8).  Explicit intrinsics: no FMA contraction across cells.
+__device__ __forceinline__ void cell_split_flux(const float (&u)[NCOMP], const GasConst& gc, float (&gr)[NCOMP],
+                                                float (&gl)[NCOMP]) {
+    const float rinv = rcp_fast(u[0]);
+    const float v = __fmul_rn(u[1], rinv);
+    float q = __fmul_rn(u[2], u[2]);
+    q = fmaf(u[3], u[3], q);
+    q = fmaf(u[1], u[1], q);
+    const float hk = __fmul_rn(0.5f, rinv);
+    const float eint = fmaf(-q, hk, u[4]);
+    const float P = __fmul_rn(gc.gm1, eint);
+    const float cs = sqrt_fast(__fmul_rn(__fmul_rn(gc.ggm1, eint), rinv));
+    const float c = __fadd_rn(fabsf(v), cs);
+    const float cp = __fadd_rn(c, v), cm = __fsub_rn(c, v);
+    const float Pv = __fmul_rn(P, v);
+    gr[0] = __fmul_rn(u[0], cp);
+    gr[1] = fmaf(u[1], cp, P);
+    gr[2] = __fmul_rn(u[2], cp);
+    gr[3] = __fmul_rn(u[3], cp);
+    gr[4] = fmaf(u[4], cp, Pv);
+    gl[0] = __fmul_rn(u[0], cm);
+    gl[1] = fmaf(u[1], cm, -P);
+    gl[2] = __fmul_rn(u[2], cm);
+    gl[3] = __fmul_rn(u[3], cm);
+    gl[4] = fmaf(u[4], cm, -Pv);
+}
+
+// base + a b / (a + b) if a b > 0, else base     (sgn = +1)   |   base - a b / (a + b) ...   (sgn = -1)
+// A select on the sign of the product, never a mask (reading R6).
+template <int SGN>
+__device__ __forceinline__ float limited(float base, float a, float b) {
+    const float p = a * b;
+    const float r = rcp_fast(a + b);
+    const float x = fmaf(SGN > 0 ? p : -p, r, base);
+    return p > 0.f ? x : base;
+}
+
+// Marches one row.  `src[q]` points to cell 0 of component q (row-local order), element n at src[q][n * STRIDE].
+// Sink must provide:
+//   template <int ODD> void cell(int j, const float (&u)[5])   updated cell j = 3..18 (ODD = j & 1, static),
+//                                            row-local component order
+//   void face(int p, const float (&f)[5])   true flux F^{t+dt/2} through interface 2|3 (p=0), 10|11 (1), 18|19 (2);
+//                                            called only if WANT_FACE
+// A Sink may overwrite the row in place at index j (the march never reads cell j again).
+//
+// The march is a software pipeline: at step n it loads cell n, forms the half-step coefficients of cell n, the
+// midpoint state of cell m = n-1 and its G^R, G^L, the right-moving limited flux through (m-1|m), the left-moving one
+// through (m-2|m-1), the total flux through (m-2|m-1) and the new value of cell m-2 = n-3.  Steps 0..5 fill the
+// pipeline (PH = n, statically pruned); steps 6..21 are identical and run as a rolled loop (PH = 6) so that the code
+// of all three sweeps stays resident in the instruction cache.
+template <int STRIDE, bool WANT_FACE, class Sink>
+struct RowMarch {
+    float u1[NCOMP], u2[NCOMP], u3[NCOMP];     // u_{n-1}, u_{n-2}, u_{n-3} (the originals, kept for Eqs.13-14)
+    float sig1;                                // 1 - 2 q c of cell n-1
+    float cp1, P1, Pv1;                        // q (c+v), q P, q P v of cell n-1
+    float cp2, P2, Pv2;                        // ... of cell n-2
+    float gr2_prev[NCOMP], gl2_prev[NCOMP];    // midpoint G^R, G^L of cell m-1
+    float ar1[NCOMP], al1[NCOMP];              // G^R_{m-1} - G^R_{m-2}, G^L_{m-1} - G^L_{m-2}
+    float xr_prev[NCOMP];                      // 2 F^R through (m-2|m-1), limited
+    float fh_prev[NCOMP];                      // 2 F^h through (m-3|m-2)
+
+    template <int PH>
+    __device__ __forceinline__ void step(const float (&u)[NCOMP], int n, const GasConst& gc, Sink& sink) {
+        const HalfCoef h = half_coef(u, gc);                                // (a), cell n
+        if (PH >= 2) {                                                      // midpoint cell m = n-1: (b)+(c)
+            float uh[NCOMP], gr2[NCOMP], gl2[NCOMP];
+            const float dP = __fsub_rn(P2, h.P), dPv = __fsub_rn(Pv2, h.Pv);
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                float b = (k == 1) ? fmaf(sig1, u1[k], dP) : ((k == 4) ? fmaf(sig1, u1[k], dPv) : __fmul_rn(sig1, u1[k]));
+                b = fmaf(cp2, u2[k], b);
+                uh[k] = fmaf(h.cm, u[k], b);
+            }
+            cell_split_flux(uh, gc, gr2, gl2);                              // (d)
+            if (PH >= 3) {                                                  // m >= 2
+                float ar0[NCOMP], al0[NCOMP];
+#pragma unroll
+                for (int k = 0; k < NCOMP; ++k) {
+                    ar0[k] = gr2[k] - gr2_prev[k];                          // G^R_m - G^R_{m-1}
+                    al0[k] = gl2[k] - gl2_prev[k];                          // G^L_m - G^L_{m-1}
+                }
+                float xr[NCOMP];
+                if (PH >= 4) {                                              // m >= 3: (e) right-moving, (m-1|m)
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) xr[k] = limited<+1>(gr2_prev[k], ar1[k], ar0[k]);
+                }
+                if (PH >= 5) {                                              // m >= 4: (e) left-moving, (m-2|m-1)
+                    float fh[NCOMP];
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) {
+                        // a = G^L_{m-1}-G^L_m = -al0, b = G^L_{m-2}-G^L_{m-1} = -al1: a b = al0 al1, a+b = -(al0+al1)
+                        const float xl = limited<-1>(gl2_prev[k], al0[k], al1[k]);
+                        fh[k] = xr_prev[k] - xl;
+                    }
+                    if (WANT_FACE) {
+                        const int i = n - 3;                                // interface (i | i+1), i = m-2
+                        if (i == NG - 1 || i == NG + PS / 2 - 1 || i == NG + PS - 1) {
+                            float ff[NCOMP];
+#pragma unroll
+                            for (int k = 0; k < NCOMP; ++k) ff[k] = 0.5f * fh[k];
+                            sink.face(i == NG - 1 ? 0 : (i == NG + PS - 1 ? 2 : 1), ff);
+                        }
+                    }
+                    if (PH >= 6) {                                          // m >= 5: (f) cell j = m-2 = n-3
+                        float un[NCOMP];
+#pragma unroll
+                        for (int k = 0; k < NCOMP; ++k) un[k] = fmaf(-gc.kh, fh[k] - fh_prev[k], u3[k]);
+                        sink.template cell<(PH + 1) & 1>(n - 3, un);        // parity of j = n-3 is static
+                    }
+#pragma unroll
+                    for (int k = 0; k < NCOMP; ++k) fh_prev[k] = fh[k];
+                }
+#pragma unroll
+                for (int k = 0; k < NCOMP; ++k) {
+                    if (PH >= 4) xr_prev[k] = xr[k];
+                    ar1[k] = ar0[k];
+                    al1[k] = al0[k];
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                gr2_prev[k] = gr2[k];
+                gl2_prev[k] = gl2[k];
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NCOMP; ++k) {
+            if (PH >= 2) u3[k] = u2[k];
+            if (PH >= 1) u2[k] = u1[k];
+            u1[k] = u[k];
+        }
+        if (PH >= 1) { cp2 = cp1; P2 = P1; Pv2 = Pv1; }
+        cp1 = h.cp; P1 = h.P; Pv1 = h.Pv; sig1 = h.sig;
+    }
+
+    // Cells are fetched two at a time (n even, n+1): a row along x is read with 64-bit shared-memory loads.
+    template <int PH0, int PH1>
+    __device__ __forceinline__ void pair(const float* const (&src)[NCOMP], int n, const GasConst& gc, Sink& sink) {
+        float ua[NCOMP], ub[NCOMP];
+        if (STRIDE == 1) {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                const float2 t = *reinterpret_cast<const float2*>(src[k] + n);
+                ua[k] = t.x;
+                ub[k] = t.y;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                ua[k] = src[k][n * STRIDE];
+                ub[k] = src[k][(n + 1) * STRIDE];
+            }
+        }
+        step<PH0>(ua, n, gc, sink);
+        step<PH1>(ub, n + 1, gc, sink);
+    }
+
+    __device__ __forceinline__ void run(const float* const (&src)[NCOMP], const GasConst& gc, Sink& sink) {
+        pair<0, 1>(src, 0, gc, sink);
+        pair<2, 3>(src, 2, gc, sink);
+        pair<4, 5>(src, 4, gc, sink);
+#pragma unroll MARCH_UNROLL
+        for (int n = 6; n < NP; n += 2) pair<6, 6>(src, n, gc, sink);
+    }
+};
+
+template <int STRIDE, bool WANT_FACE, class Sink>
+__device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], const GasConst& gc, Sink& sink) {
+    RowMarch<STRIDE, WANT_FACE, Sink> m;
+    m.run(src, gc, sink);
+}
+
+}  // namespace gamer
