@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "gamer_hydro.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("hydro_kernel.cuh", "rtvd_march.cuh")] + \
+DEPS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))] + \
     [os.path.join(os.path.dirname(HERE), "include", "gamer_hydro.h")]
 LIB = os.path.join(HERE, "libgamer_hydro.so")
 
@@ -24,15 +24,17 @@ def nvcc():
     return "nvcc"
 
 
-def build(force=False, verbose=False, extra=()):
-    if (not force) and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
-        return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + list(extra) + ["-o", LIB + ".tmp"] + SOURCES
+def build(force=False, verbose=False, extra=(), out=None):
+    """Compile the library to `out` (default: the in-tree libgamer_hydro.so); `extra` = more nvcc flags."""
+    lib = out or LIB
+    if (not force) and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in DEPS):
+        return lib
+    cmd = [nvcc()] + NVCC_FLAGS + list(extra) + ["-o", lib + ".tmp"] + SOURCES
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
-    return LIB
+    os.replace(lib + ".tmp", lib)
+    return lib
 
 
 if __name__ == "__main__":

@@ -46,13 +46,13 @@ KernelFn pick_kernel(bool backward, bool face, bool speed) {
 struct DeviceInfo {
     bool ready = false;
     int sm_count = 0;
-    bool attr_set[8] = {false, false, false, false, false, false, false, false};
+    bool attr_set[16] = {};
 };
 std::mutex g_mu;
 DeviceInfo g_dev[64];
 
 // SM count of the current device and the opt-in to 208 KB of dynamic shared memory, once per device and kernel.
-int prepare(KernelFn fn, int key, int* sm_count) {
+int prepare(const void* fn, int key, int smem_bytes, int* sm_count) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
@@ -74,8 +74,7 @@ int prepare(KernelFn fn, int key, int* sm_count) {
         di.ready = true;
     }
     if (!di.attr_set[key]) {
-        e = cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 gamer::SMEM_BYTES);
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
         if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         di.attr_set[key] = true;
     }
@@ -113,9 +112,9 @@ gamer::GasConst make_const(float dt, float dh, float gamma) {
 int launch(const float* d_in, float* d_out, long long n_groups, float dt, float dh, float gamma, int backward,
            float* d_face, float* d_speed, cudaStream_t stream) {
     const int key = (backward ? 4 : 0) | (d_face ? 2 : 0) | (d_speed ? 1 : 0);
-    KernelFn fn = pick_kernel(backward != 0, d_face != nullptr, d_speed != nullptr);
     int sm_count = 0;
-    const int rc = prepare(fn, key, &sm_count);
+    KernelFn fn = pick_kernel(backward != 0, d_face != nullptr, d_speed != nullptr);
+    const int rc = prepare(reinterpret_cast<const void*>(fn), key, gamer::SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
     const int grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
     fn<<<grid, gamer::BLOCK_THREADS, gamer::SMEM_BYTES, stream>>>(d_in, d_out, n_groups, make_const(dt, dh, gamma),
@@ -214,21 +213,29 @@ int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups
 }
 
 int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread) {
-    KernelFn fn = pick_kernel(false, false, false);
+    const void* fn = reinterpret_cast<const void*>(pick_kernel(false, false, false));
+    const int smem = gamer::SMEM_BYTES;
     int sm_count = 0;
-    const int rc = prepare(fn, 0, &sm_count);
+    const int rc = prepare(fn, 0, smem, &sm_count);
     if (rc != GAMER_OK) return rc;
     cudaFuncAttributes fa;
-    const cudaError_t e = cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn));
+    const cudaError_t e = cudaFuncGetAttributes(&fa, fn);
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaFuncGetAttributes: %s", cudaGetErrorString(e));
     if (n_groups < 0) n_groups = 0;
     if (grid) *grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
     if (block) *block = gamer::BLOCK_THREADS;
-    if (smem_bytes) *smem_bytes = gamer::SMEM_BYTES;
+    if (smem_bytes) *smem_bytes = smem;
     if (regs_per_thread) *regs_per_thread = fa.numRegs;
     g_err[0] = '\0';
     return GAMER_OK;
 }
+
+#ifdef GAMER_PHASE_TIMERS
+// debug builds only (never defined by build.py): per-CTA cycles {wait for planes, x, y, z} of the last launch
+GAMER_API int gamer_debug_phase_cycles(long long* host, int n_ctas) {
+    return (int)cudaMemcpyFromSymbol(host, gamer::g_phase_cycles, sizeof(long long) * 4 * (size_t)n_ctas);
+}
+#endif
 
 const char* gamer_last_error(void) { return g_err; }
 const char* gamer_version(void) { return "gamer-hydro-b200 0.1.0 (sm_100a)"; }

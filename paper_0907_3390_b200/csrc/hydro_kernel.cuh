@@ -1,18 +1,16 @@
 // hydro_kernel.cuh — the batched hydro kernel (sm_100a): one persistent CTA per SM, one patch group at a time.
 //
 // Per group (steps 1-10):
-//   H0  one elected thread bulk-copies the padded group (212 960 B, contiguous in HBM) into shared memory with
-//       cp.async.bulk (TMA, SASS UBLKCP) completing on an mbarrier; the next group is prefetched into L2 meanwhile
+//   H0  the padded group (212 960 B, contiguous in HBM) is bulk-copied into shared memory with cp.async.bulk (TMA,
+//       SASS UBLKCP) completing on mbarriers.  Forward pass: in three chunks of z-planes, each issued by a warp
+//       without z rows as soon as the z sweep of the PREVIOUS group has read those planes (the load runs under the
+//       z sweep).  Backward pass: one copy per group, the next group prefetched into L2 meanwhile.
 //   H1-H7 three in-place sweeps, one thread per row (rtvd_march), rows shrinking 22x22 -> 16x22 -> 16x16
 //   H9  the last sweep streams the 16^3 interior to HBM (forward: straight from the registers of the z march,
 //       64-byte segments; backward: in place, then a 128-bit coalesced copy-out)
 #pragma once
 #include <cstdint>
-#ifdef GAMER_MARCH_V1
 #include "rtvd_march.cuh"
-#else
-#include "rtvd_march2.cuh"
-#endif
 
 namespace gamer {
 
@@ -25,7 +23,8 @@ constexpr int GROUP_OUT_FLOATS = NCOMP * PS * PS * PS;    // 20 480
 constexpr int GROUP_FACE_FLOATS = 3 * 3 * NCOMP * PS * PS;
 constexpr int GROUP_IN_BYTES = GROUP_IN_FLOATS * 4;       // 212 960
 constexpr int VAR_FLOATS = NP * NP * NP;                  // 10 648
-constexpr int SMEM_BYTES = GROUP_IN_BYTES + 64;           // + mbarrier and reduction scratch
+constexpr int CTL_BYTES = 512;                            // mbarriers, counters, reduction scratch (struct Ctl)
+constexpr int SMEM_BYTES = GROUP_IN_BYTES + CTL_BYTES;
 
 #ifdef GAMER_PHASE_TIMERS
 // debug builds only (never defined by build.py): per-CTA cycles spent waiting for the load / in each sweep
@@ -172,9 +171,11 @@ __device__ __forceinline__ int var_of(int d, int q) {
 
 // One sweep along axis D over the rows that are still valid.  `smem` holds the group as [v][z][y][x].
 //   LO_A/N_A, LO_B/N_B: the two transverse axes (A = lower axis number, fastest across threads), start and count.
-template <int D, int LO_A, int N_A, int LO_B, int N_B, bool LAST, bool LAST_TO_GLOBAL, bool WANT_FACE, bool WANT_SPEED>
+//   t: index of this thread's row among the N_A * N_B rows (rows beyond are skipped).  gate: see RowMarch::pair.
+template <int D, int LO_A, int N_A, int LO_B, int N_B, bool LAST, bool LAST_TO_GLOBAL, bool WANT_FACE, bool WANT_SPEED,
+          class Gate>
 __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __restrict__ out_g,
-                                      float* __restrict__ face_g, float& speed) {
+                                      float* __restrict__ face_g, float& speed, const int t, Gate& gate) {
     constexpr int STRIDE = D == 0 ? 1 : (D == 1 ? NP : NP * NP);
     constexpr int AX_A = D == 0 ? 1 : 0;                      // transverse axes: the two that are not D, ascending
     constexpr int AX_B = D == 2 ? 1 : 2;
@@ -183,12 +184,7 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
     constexpr int OSTRIDE = D == 0 ? 1 : (D == 1 ? PS : PS * PS);
     constexpr int OSTR_A = AX_A == 0 ? 1 : PS;
     constexpr int OSTR_B = AX_B == 1 ? PS : PS * PS;
-#ifdef GAMER_DUP_ROWS      // timing experiment only: surplus threads redo rows (results are garbage)
-    const int t = threadIdx.x % (N_A * N_B);
-#else
-    const int t = threadIdx.x;
     if (t >= N_A * N_B) return;
-#endif
     // padded transverse coordinates of this thread's row.  Where the fast axis is the 16 interior x cells, the two
     // half-warps are placed 16 banks apart (y sweep: z and z+4; z sweep: y and y+8) so that the 4-byte accesses of a
     // warp hit 32 different banks; rows along x are 8-byte accessed and conflict-free for consecutive rows.
@@ -218,7 +214,7 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
                                      : nullptr;
         }
         sink.face_row = face_row;
-        rtvd_march<STRIDE, WANT_FACE>(src, gc, sink);
+        rtvd_march<STRIDE, WANT_FACE>(src, gc, sink, gate);
     } else {
         FinalSink<STRIDE, OSTRIDE, LAST_TO_GLOBAL, WANT_SPEED> sink;
 #pragma unroll
@@ -233,8 +229,99 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
         sink.gm1 = gc.gm1;
         sink.ggm1 = gc.ggm1;
         sink.speed = speed;
-        rtvd_march<STRIDE, WANT_FACE>(src, gc, sink);
+        rtvd_march<STRIDE, WANT_FACE>(src, gc, sink, gate);
         speed = sink.speed;
+    }
+}
+
+// ---- control block behind the group in shared memory -------------------------------------------------------------
+constexpr int PLANE_FLOATS = NP * NP;             // 484: one z-plane of one variable, contiguous in HBM and in smem
+constexpr int PLANE_BYTES = PLANE_FLOATS * 4;     // 1936 = 16 * 121
+constexpr int N_ZPAIR = NP / 2;                   // 11 pairs of z-planes
+constexpr int N_ZWARP = PS * PS / 32;             // 8 warps march along z
+
+#ifndef GAMER_CHUNK_PAIRS
+#define GAMER_CHUNK_PAIRS 4           /* z-plane pairs per load chunk: planes 0-7, 8-15, 16-21 */
+#endif
+constexpr int CHUNK_PAIRS = GAMER_CHUNK_PAIRS;
+constexpr int N_CHUNK = (N_ZPAIR + CHUNK_PAIRS - 1) / CHUNK_PAIRS;
+__host__ __device__ constexpr int chunk_of_plane(int z) { return (z >> 1) / CHUNK_PAIRS; }
+__host__ __device__ constexpr int chunk_lo(int c) { return 2 * c * CHUNK_PAIRS; }                    // first plane
+__host__ __device__ constexpr int chunk_hi(int c) {                                                  // one past last
+    return 2 * (c + 1) * CHUNK_PAIRS < NP ? 2 * (c + 1) * CHUNK_PAIRS : NP;
+}
+
+struct Ctl {
+    uint64_t full[N_ZPAIR];           // forward: load chunk c of the group has landed; backward: full[0] = whole group
+    uint64_t zfree[N_ZPAIR];          // forward: all 256 z threads have planes 2k, 2k+1 in registers
+    unsigned int red[4];              // CFL speed of the group (bit pattern), slot = iteration & 3
+    unsigned int zfin[4];             // warps that have finished the group, slot = iteration & 3
+};
+static_assert(sizeof(Ctl) <= CTL_BYTES, "control block");
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// Waits with a suspend-time hint: the hardware parks the warp until the phase completes instead of polling.
+__device__ __forceinline__ void mbar_wait_parked(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity), "r"(1000000u)
+            : "memory");
+    } while (!ok);
+}
+
+// Bulk copies (TMA) of load chunk c — z-planes chunk_lo(c)..chunk_hi(c)-1, contiguous per variable in HBM and in
+// shared memory — of all five variables of one group; they complete on full[c].  One thread calls this.
+__device__ __forceinline__ void load_chunk(float* smem, Ctl* ctl, const float* __restrict__ in_g, int c) {
+    const int lo = chunk_lo(c), bytes = (chunk_hi(c) - lo) * PLANE_BYTES;
+    mbar_expect_tx(&ctl->full[c], NCOMP * bytes);
+#pragma unroll
+    for (int v = 0; v < NCOMP; ++v)
+        bulk_g2s(smem + v * VAR_FLOATS + lo * PLANE_FLOATS, in_g + v * VAR_FLOATS + lo * PLANE_FLOATS, bytes,
+                 &ctl->full[c]);
+}
+
+// Gate of the forward z march (the last sweep; its results go straight to HBM): once a thread has planes n, n+1 in
+// registers it never reads them again and says so on zfree[n/2] (fire and forget: nothing in the march waits).  A
+// warp without z rows waits for these barriers and starts the bulk copies of the same planes of the CTA's NEXT group
+// into the space (load_next_group), so that the load runs under the z sweep instead of in front of the x sweep.
+struct ZPlaneGate {
+    Ctl* ctl;
+    __device__ __forceinline__ void acquire(int) {}
+    __device__ __forceinline__ void release(int n) { mbar_arrive(&ctl->zfree[n >> 1]); }
+};
+
+// Called by one thread during the z sweep of the group of iteration `it`.
+__device__ __forceinline__ void load_next_group(float* smem, Ctl* ctl, const float* __restrict__ in_next, unsigned int it) {
+    for (int c = 0; c < N_CHUNK; ++c) {
+        mbar_wait_parked(&ctl->zfree[chunk_hi(c) / 2 - 1], it & 1u);   // z warps pass the pairs in order
+        fence_proxy_async();
+        load_chunk(smem, ctl, in_next, c);
+    }
+}
+
+// Per-group CFL speed: warp maximum, then a shared-memory maximum over the warps that hold final cells; the last of
+// them writes group_maxspeed[g].  The slot (iteration & 3) keeps groups that overlap in time apart.
+__device__ __forceinline__ void reduce_speed(Ctl* ctl, float speed, unsigned int it, int n_warps,
+                                             float* __restrict__ dst) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) speed = fmaxf(speed, __shfl_xor_sync(0xffffffffu, speed, o));
+    if ((threadIdx.x & 31) == 0) {
+        const int slot = it & 3;
+        atomicMax(&ctl->red[slot], __float_as_uint(speed));          // positive floats order like their bit patterns
+        if (atomicAdd(&ctl->zfin[slot], 1u) == (unsigned int)(n_warps - 1)) {
+            *dst = __uint_as_float(atomicExch(&ctl->red[slot], 0u));
+            ctl->zfin[slot] = 0u;
+        }
     }
 }
 
@@ -244,13 +331,24 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
                      float* __restrict__ face_flux, float* __restrict__ group_maxspeed) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* smem = reinterpret_cast<float*>(smem_raw);
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + GROUP_IN_BYTES);
-    unsigned int* red = reinterpret_cast<unsigned int*>(smem_raw + GROUP_IN_BYTES + 16);
+    Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + GROUP_IN_BYTES);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
-        mbar_init(bar, 1);
-        *red = 0u;
+        for (int k = 0; k < N_ZPAIR; ++k) {
+            mbar_init(&ctl->full[k], 1);
+            mbar_init(&ctl->zfree[k], PS * PS);
+        }
+        for (int i = 0; i < 4; ++i) {
+            ctl->red[i] = 0u;
+            ctl->zfin[i] = 0u;
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (!BACKWARD) {              // the first group of this CTA, plane by plane
+            fence_proxy_async();
+            const float* in_g = in + (long long)blockIdx.x * GROUP_IN_FLOATS;
+            for (int c = 0; c < N_CHUNK; ++c) load_chunk(smem, ctl, in_g, c);
+        }
     }
     __syncthreads();
 
@@ -262,37 +360,61 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
 #define PHASE_T0()
 #define PHASE_ACC(i)
 #endif
-    uint32_t parity = 0;
-    for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
-        PHASE_T0();
-        if (threadIdx.x == 0) {
-            fence_proxy_async();      // generic-proxy accesses of the previous group are ordered before the async write
-            mbar_expect_tx(bar, GROUP_IN_BYTES);
-            bulk_g2s(smem, in + g * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES, bar);
-            const long long gn = g + gridDim.x;
-            if (gn < n_groups) bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES);
-        }
-        mbar_wait(bar, parity);
-        parity ^= 1u;
-        PHASE_ACC(0);
-
+    NoGate nogate;
+    unsigned int it = 0;
+    for (long long g = blockIdx.x; g < n_groups; g += gridDim.x, ++it) {
+        const uint32_t parity = it & 1u;
         float* out_g = out + g * (long long)GROUP_OUT_FLOATS;
         float* face_g = WANT_FACE ? face_flux + g * (long long)GROUP_FACE_FLOATS : nullptr;
         float speed = 0.f;
+        PHASE_T0();
         if (!BACKWARD) {
-            sweep<0, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);   // x: (y,z) all
+            // x sweep: warp w takes the (z,y) rows 32w..32w+31 and starts as soon as their planes have landed.  Warps
+            // 8..15 have no z rows and arrive here while the z sweep of the previous group is still running.
+            // (Giving those warps the planes that are handed back first was measured: no gain.)
+            const int row_lo = 32 * warp, row_hi = row_lo + 31 < NP * NP ? row_lo + 31 : NP * NP - 1;
+            for (int c = chunk_of_plane(row_lo / NP); c <= chunk_of_plane(row_hi / NP); ++c)
+                mbar_wait_parked(&ctl->full[c], parity);
+            PHASE_ACC(0);
+            sweep<0, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, row_lo + lane, nogate);
             __syncthreads();
             PHASE_ACC(1);
-            sweep<1, NG, PS, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);  // y: x int, z all
+            sweep<1, NG, PS, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
             PHASE_ACC(2);
-            sweep<2, NG, PS, NG, PS, true, true, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed);   // z
+            const long long gn = g + gridDim.x;
+            if (warp < N_ZWARP) {
+                ZPlaneGate gate;
+                gate.ctl = ctl;
+                sweep<2, NG, PS, NG, PS, true, true, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
+                                                                            gate);
+                if (WANT_SPEED) reduce_speed(ctl, speed, it, N_ZWARP, group_maxspeed + g);
+            } else if (threadIdx.x == BLOCK_THREADS - 32 && gn < n_groups) {
+                load_next_group(smem, ctl, in + gn * (long long)GROUP_IN_FLOATS, it);
+            }
+            PHASE_ACC(3);
+            // no CTA-wide barrier: a plane is overwritten only after all z threads have read it (zfree[]), and the
+            // next group's x tasks wait for full[] of their planes
         } else {
-            sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);   // z: (x,y) all
+            uint64_t* bar = &ctl->full[0];
+            if (threadIdx.x == 0) {
+                fence_proxy_async();  // generic-proxy accesses of the previous group are ordered before the async write
+                mbar_expect_tx(bar, GROUP_IN_BYTES);
+                bulk_g2s(smem, in + g * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES, bar);
+                const long long gn = g + gridDim.x;
+                if (gn < n_groups) bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES);
+            }
+            mbar_wait_parked(bar, parity);
+            PHASE_ACC(0);
+            sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
-            sweep<1, 0, NP, NG, PS, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed);  // y: x all, z int
+            PHASE_ACC(1);
+            sweep<1, 0, NP, NG, PS, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
-            sweep<0, NG, PS, NG, PS, true, false, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed);  // x in place
+            PHASE_ACC(2);
+            sweep<0, NG, PS, NG, PS, true, false, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
+                                                                         nogate);
+            if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);
             __syncthreads();
             // coalesced 128-bit copy-out of the interior: 16 B = 4 cells of a 16-cell row (row start 3 is not 16-B
             // aligned in shared memory, so read scalars, write float4)
@@ -302,20 +424,9 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
                 float4 val = make_float4(s[0], s[1], s[2], s[3]);
                 reinterpret_cast<float4*>(out_g)[i] = val;
             }
+            __syncthreads();          // every thread is done with the buffer before the next bulk copy overwrites it
+            PHASE_ACC(3);
         }
-        if (WANT_SPEED) {
-            // positive floats order like their bit patterns
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) speed = fmaxf(speed, __shfl_xor_sync(0xffffffffu, speed, o));
-            if ((threadIdx.x & 31) == 0) atomicMax(red, __float_as_uint(speed));
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                group_maxspeed[g] = __uint_as_float(*red);
-                *red = 0u;
-            }
-        }
-        __syncthreads();     // every thread is done with the buffer before the next bulk copy overwrites it
-        PHASE_ACC(3);
     }
 #ifdef GAMER_PHASE_TIMERS
     if (threadIdx.x == 0)
