@@ -233,7 +233,7 @@ int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem
 #ifdef GAMER_PHASE_TIMERS
 // debug builds only (never defined by build.py): per-CTA cycles {wait for planes, x, y, z} of the last launch
 GAMER_API int gamer_debug_phase_cycles(long long* host, int n_ctas) {
-    return (int)cudaMemcpyFromSymbol(host, gamer::g_phase_cycles, sizeof(long long) * 4 * (size_t)n_ctas);
+    return (int)cudaMemcpyFromSymbol(host, gamer::g_phase_cycles, sizeof(long long) * 16 * 8 * (size_t)n_ctas);
 }
 #endif
 

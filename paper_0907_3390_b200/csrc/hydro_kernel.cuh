@@ -28,7 +28,7 @@ constexpr int SMEM_BYTES = GROUP_IN_BYTES + CTL_BYTES;
 
 #ifdef GAMER_PHASE_TIMERS
 // debug builds only (never defined by build.py): per-CTA cycles spent waiting for the load / in each sweep
-__device__ long long g_phase_cycles[1024 * 4];
+__device__ long long g_phase_cycles[160 * 16 * 8];   // [cta][warp][slot]
 #endif
 
 // ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------------------
@@ -253,30 +253,52 @@ __host__ __device__ constexpr int chunk_hi(int c) {                             
 
 struct Ctl {
     uint64_t full[N_ZPAIR];           // forward: load chunk c of the group has landed; backward: full[0] = whole group
-    uint64_t zfree[N_ZPAIR];          // forward: all 256 z threads have planes 2k, 2k+1 in registers
     unsigned int red[4];              // CFL speed of the group (bit pattern), slot = iteration & 3
     unsigned int zfin[4];             // warps that have finished the group, slot = iteration & 3
 };
 static_assert(sizeof(Ctl) <= CTL_BYTES, "control block");
 
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
-// Waits with a suspend-time hint: the hardware parks the warp until the phase completes instead of polling.
-__device__ __forceinline__ void mbar_wait_parked(uint64_t* bar, uint32_t parity) {
+// Polls an mbarrier phase.  try_wait comes back after a few cycles whatever suspend-time hint it is given (measured:
+// one poll per ~13 cycles), and a polling warp takes issue slots from the marching warps of its SM sub-partition — the
+// z warps that shared one with pollers ran 30 % slower.  So only ONE warp ever polls (the loader); every other wait
+// in the forward pass is a hardware named barrier (bar.sync blocks without issuing).
+__device__ __forceinline__ void mbar_wait_poll(uint64_t* bar, uint32_t parity) {
     uint32_t ok;
     do {
         asm volatile(
             "{\n"
             ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
             "selp.u32 %0, 1, 0, p;\n"
             "}\n"
             : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity), "r"(1000000u)
+            : "r"(smem_u32(bar)), "r"(parity)
             : "memory");
     } while (!ok);
+}
+__device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n_threads) : "memory");
+}
+__device__ __forceinline__ void named_bar_arrive(int id, int n_threads) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n_threads) : "memory");
+}
+
+// Named barriers of the forward pass (0 is __syncthreads).  LOADER_WARP has no z rows and only 4 x rows.
+constexpr int LOADER_WARP = BLOCK_THREADS / 32 - 1;
+constexpr int BAR_ZFREE = 1;                      // + c: the 256 z threads arrive, the loader warp syncs
+constexpr int BAR_FULL = 1 + N_CHUNK;             // + c: the loader warp arrives, the x warps that need chunk c sync
+static_assert(BAR_FULL + N_CHUNK <= 16, "named barriers");
+constexpr int ZFREE_THREADS = PS * PS + 32;
+// first / last load chunk that the x task of warp w (rows 32w..32w+31 of the (z,y) rows) reads
+__host__ __device__ constexpr int xtask_chunk_lo(int w) { return chunk_of_plane(32 * w / NP); }
+__host__ __device__ constexpr int xtask_chunk_hi(int w) {
+    return chunk_of_plane((32 * w + 31 < NP * NP ? 32 * w + 31 : NP * NP - 1) / NP);
+}
+__host__ __device__ constexpr int full_threads(int c) {       // participants of BAR_FULL + c
+    int n = 32;                                               // the loader
+    for (int w = 0; w < LOADER_WARP; ++w)
+        if (xtask_chunk_lo(w) <= c && c <= xtask_chunk_hi(w)) n += 32;
+    return n;
 }
 
 // Bulk copies (TMA) of load chunk c — z-planes chunk_lo(c)..chunk_hi(c)-1, contiguous per variable in HBM and in
@@ -290,22 +312,38 @@ __device__ __forceinline__ void load_chunk(float* smem, Ctl* ctl, const float* _
                  &ctl->full[c]);
 }
 
-// Gate of the forward z march (the last sweep; its results go straight to HBM): once a thread has planes n, n+1 in
-// registers it never reads them again and says so on zfree[n/2] (fire and forget: nothing in the march waits).  A
-// warp without z rows waits for these barriers and starts the bulk copies of the same planes of the CTA's NEXT group
-// into the space (load_next_group), so that the load runs under the z sweep instead of in front of the x sweep.
+// Gate of the forward z march (the last sweep; its results go straight to HBM): once a thread has the last planes of
+// a load chunk in registers it never reads the chunk again and says so on BAR_ZFREE + c (bar.arrive: nothing in the
+// march waits).  The loader warp syncs on these barriers and starts the bulk copies of the same planes of the CTA's
+// NEXT group into the space, so that the load runs under the z sweep instead of in front of the x sweep.
 struct ZPlaneGate {
-    Ctl* ctl;
+    bool has_next;
     __device__ __forceinline__ void acquire(int) {}
-    __device__ __forceinline__ void release(int n) { mbar_arrive(&ctl->zfree[n >> 1]); }
+    __device__ __forceinline__ void release(int n) {
+        const int k = n >> 1;
+        if (has_next && ((k + 1) % CHUNK_PAIRS == 0 || k == N_ZPAIR - 1))
+            named_bar_arrive(BAR_ZFREE + k / CHUNK_PAIRS, ZFREE_THREADS);
+    }
 };
 
-// Called by one thread during the z sweep of the group of iteration `it`.
-__device__ __forceinline__ void load_next_group(float* smem, Ctl* ctl, const float* __restrict__ in_next, unsigned int it) {
+// The loader warp, during the z sweep of a group that has a successor.
+__device__ __forceinline__ void load_next_group(float* smem, Ctl* ctl, const float* __restrict__ in_next) {
+#pragma unroll
     for (int c = 0; c < N_CHUNK; ++c) {
-        mbar_wait_parked(&ctl->zfree[chunk_hi(c) / 2 - 1], it & 1u);   // z warps pass the pairs in order
-        fence_proxy_async();
-        load_chunk(smem, ctl, in_next, c);
+        named_bar_sync(BAR_ZFREE + c, ZFREE_THREADS);
+        if ((threadIdx.x & 31) == 0) {
+            fence_proxy_async();
+            load_chunk(smem, ctl, in_next, c);
+        }
+    }
+}
+
+// The loader warp, before the x sweep: tells the x warps which chunks have landed.
+__device__ __forceinline__ void release_chunks(Ctl* ctl, uint32_t parity) {
+#pragma unroll
+    for (int c = 0; c < N_CHUNK; ++c) {
+        mbar_wait_poll(&ctl->full[c], parity);
+        named_bar_arrive(BAR_FULL + c, full_threads(c));
     }
 }
 
@@ -335,10 +373,7 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
-        for (int k = 0; k < N_ZPAIR; ++k) {
-            mbar_init(&ctl->full[k], 1);
-            mbar_init(&ctl->zfree[k], PS * PS);
-        }
+        for (int k = 0; k < N_ZPAIR; ++k) mbar_init(&ctl->full[k], 1);
         for (int i = 0; i < 4; ++i) {
             ctl->red[i] = 0u;
             ctl->zfin[i] = 0u;
@@ -353,7 +388,7 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
     __syncthreads();
 
 #ifdef GAMER_PHASE_TIMERS
-    long long tacc[5] = {0, 0, 0, 0, 0}, tt0, tt1;
+    long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tt0, tt1;
 #define PHASE_T0() tt0 = clock64()
 #define PHASE_ACC(i) do { tt1 = clock64(); tacc[i] += tt1 - tt0; tt0 = tt1; } while (0)
 #else
@@ -372,29 +407,35 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             // x sweep: warp w takes the (z,y) rows 32w..32w+31 and starts as soon as their planes have landed.  Warps
             // 8..15 have no z rows and arrive here while the z sweep of the previous group is still running.
             // (Giving those warps the planes that are handed back first was measured: no gain.)
-            const int row_lo = 32 * warp, row_hi = row_lo + 31 < NP * NP ? row_lo + 31 : NP * NP - 1;
-            for (int c = chunk_of_plane(row_lo / NP); c <= chunk_of_plane(row_hi / NP); ++c)
-                mbar_wait_parked(&ctl->full[c], parity);
+            const int row_lo = 32 * warp;
+            if (warp == LOADER_WARP) {
+                release_chunks(ctl, parity);
+            } else {
+                for (int c = xtask_chunk_lo(warp); c <= xtask_chunk_hi(warp); ++c)
+                    named_bar_sync(BAR_FULL + c, full_threads(c));
+            }
             PHASE_ACC(0);
             sweep<0, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, row_lo + lane, nogate);
-            __syncthreads();
             PHASE_ACC(1);
-            sweep<1, NG, PS, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
+            PHASE_ACC(4);
+            sweep<1, NG, PS, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             PHASE_ACC(2);
+            __syncthreads();
+            PHASE_ACC(5);
             const long long gn = g + gridDim.x;
             if (warp < N_ZWARP) {
                 ZPlaneGate gate;
-                gate.ctl = ctl;
+                gate.has_next = gn < n_groups;
                 sweep<2, NG, PS, NG, PS, true, true, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
                                                                             gate);
                 if (WANT_SPEED) reduce_speed(ctl, speed, it, N_ZWARP, group_maxspeed + g);
-            } else if (threadIdx.x == BLOCK_THREADS - 32 && gn < n_groups) {
-                load_next_group(smem, ctl, in + gn * (long long)GROUP_IN_FLOATS, it);
+            } else if (warp == LOADER_WARP && gn < n_groups) {
+                load_next_group(smem, ctl, in + gn * (long long)GROUP_IN_FLOATS);
             }
             PHASE_ACC(3);
-            // no CTA-wide barrier: a plane is overwritten only after all z threads have read it (zfree[]), and the
-            // next group's x tasks wait for full[] of their planes
+            // no CTA-wide barrier: a plane is overwritten only after all z threads have read it (BAR_ZFREE), and the
+            // next group's x tasks wait for their planes (BAR_FULL)
         } else {
             uint64_t* bar = &ctl->full[0];
             if (threadIdx.x == 0) {
@@ -404,7 +445,7 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
                 const long long gn = g + gridDim.x;
                 if (gn < n_groups) bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES);
             }
-            mbar_wait_parked(bar, parity);
+            mbar_wait_poll(bar, parity);
             PHASE_ACC(0);
             sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
@@ -429,8 +470,8 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
         }
     }
 #ifdef GAMER_PHASE_TIMERS
-    if (threadIdx.x == 0)
-        for (int i = 0; i < 4; ++i) g_phase_cycles[blockIdx.x * 4 + i] = tacc[i];
+    if (lane == 0)
+        for (int i = 0; i < 8; ++i) g_phase_cycles[(blockIdx.x * 16 + warp) * 8 + i] = tacc[i];
 #endif
 }
 

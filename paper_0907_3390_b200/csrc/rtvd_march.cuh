@@ -19,7 +19,7 @@
 #include <cuda_runtime.h>
 
 #ifndef GAMER_MARCH_UNROLL
-#define GAMER_MARCH_UNROLL 2     /* pairs of cells per loop body */
+#define GAMER_MARCH_UNROLL 3     /* pairs of cells per loop body (measured: 1: 113.5, 2: 105.4, 3: 104.5, 4: 108.4 ns/group) */
 #endif
 
 namespace gamer {
@@ -40,14 +40,22 @@ struct GasConst {
 };
 
 __device__ __forceinline__ float rcp_fast(float x) {
+#ifdef GAMER_EXP_NOMUFU      // timing experiment only (results are garbage)
+    return __fmul_rn(x, 1.0001f);
+#else
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
+#endif
 }
 __device__ __forceinline__ float sqrt_fast(float x) {
+#ifdef GAMER_EXP_NOMUFU
+    return __fmul_rn(x, 0.9999f);
+#else
     float r;
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
+#endif
 }
 
 // What a cell at time t contributes to the half step of its neighbours and of itself (all times q = (dt/dh)/4).
@@ -119,66 +127,63 @@ __device__ __forceinline__ float limited(float base, float a, float b) {
     return p > 0.f ? x : base;
 }
 
-// Marches one row.  `src[q]` points to cell 0 of component q (row-local order), element n at src[q][n * STRIDE].
+// Marches one row.  Src::load(n, ua, ub) fetches cells n (even) and n+1 of the row, row-local component order.
 // Sink must provide:
 //   template <int ODD> void cell(int j, const float (&u)[5])   updated cell j = 3..18 (ODD = j & 1, static),
 //                                            row-local component order
 //   void face(int p, const float (&f)[5])   true flux F^{t+dt/2} through interface 2|3 (p=0), 10|11 (1), 18|19 (2);
 //                                            called only if WANT_FACE
 // A Sink may overwrite the row in place at index j (the march never reads cell j again).
+// Gate: gate.acquire(n) is called before cells n, n+1 are read and gate.release(n) once they are in registers.
 //
-// The march is a software pipeline: at step n it loads cell n, forms the half-step coefficients of cell n, the
-// midpoint state of cell m = n-1 and its G^R, G^L, the right-moving limited flux through (m-1|m), the left-moving one
-// through (m-2|m-1), the total flux through (m-2|m-1) and the new value of cell m-2 = n-3.  Steps 0..5 fill the
-// pipeline (PH = n, statically pruned); steps 6..21 are identical and run as a rolled loop (PH = 6) so that the code
-// of all three sweeps stays resident in the instruction cache.
+// The march is a software pipeline in two independent halves per step.  Step n loads cell n and
+//   stage A: forms the half-step coefficients of cell n and the midpoint state of cell n-1, which it latches;
+//   stage B: takes the midpoint state of cell m = n-2 latched by the PREVIOUS step and forms its G^R, G^L, the
+//            right-moving limited flux through (m-1|m), the left-moving one through (m-2|m-1), the total flux through
+//            (m-2|m-1) and the new value of cell m-2 = n-4.
+// Without the latch one step is a single dependency chain (coefficients -> midpoint state -> split fluxes -> limited
+// fluxes -> new value) and a warp that shares its SM sub-partition with only one or two others (y and z sweeps)
+// cannot fill the issue slots: latching cost 5 registers and one drain step per row and gained 3.4 %.
+// Steps 0..7 fill the pipeline (PH = n, statically pruned); steps 8..21 are identical and run as a rolled loop
+// (PH = 7), so that the code stays resident in the instruction cache; a last half step drains cell 18.
 template <bool WANT_FACE, class Sink>
 struct RowMarch {
-    float u1[NCOMP], u2[NCOMP], u3[NCOMP];     // u_{n-1}, u_{n-2}, u_{n-3} (the originals, kept for Eqs.13-14)
-    float sig1;                                // 1 - 2 q c of cell n-1
-    float cp1, P1, Pv1;                        // q (c+v), q P, q P v of cell n-1
+    float u1[NCOMP], u2[NCOMP], u3[NCOMP], u4[NCOMP];   // u_{n-1} .. u_{n-4} (the originals, kept for Eqs.13-14)
+    float sig1, cp1, P1, Pv1;                  // 1 - 2 q c, q (c+v), q P, q P v of cell n-1
     float cp2, P2, Pv2;                        // ... of cell n-2
+    float uhl[NCOMP];                          // midpoint state of cell m = n-2 (latched by the previous step)
     float gr2_prev[NCOMP], gl2_prev[NCOMP];    // midpoint G^R, G^L of cell m-1
     float ar1[NCOMP], al1[NCOMP];              // G^R_{m-1} - G^R_{m-2}, G^L_{m-1} - G^L_{m-2}
     float xr_prev[NCOMP];                      // 2 F^R through (m-2|m-1), limited
     float fh_prev[NCOMP];                      // 2 F^h through (m-3|m-2)
 
-    // PH: pipeline-fill phase (statically prunes what cannot be formed yet); ODD: parity of the updated cell j = n-3
+    // stage B of step n: everything that follows from the midpoint state of cell m = n-2; new value of cell j = n-4
     template <int PH, int ODD>
-    __device__ __forceinline__ void step(const float (&u)[NCOMP], int n, const GasConst& gc, Sink& sink) {
-        const HalfCoef h = half_coef(u, gc);                                // (a), cell n
-        if (PH >= 2) {                                                      // midpoint cell m = n-1: (b)+(c)
-            float uh[NCOMP], gr2[NCOMP], gl2[NCOMP];
-            const float dP = __fsub_rn(P2, h.P), dPv = __fsub_rn(Pv2, h.Pv);
-#pragma unroll
-            for (int k = 0; k < NCOMP; ++k) {
-                float b = (k == 1) ? fmaf(sig1, u1[k], dP) : ((k == 4) ? fmaf(sig1, u1[k], dPv) : __fmul_rn(sig1, u1[k]));
-                b = fmaf(cp2, u2[k], b);
-                uh[k] = fmaf(h.cm, u[k], b);
-            }
-            cell_split_flux(uh, gc, gr2, gl2);                              // (d)
-            if (PH >= 3) {                                                  // m >= 2
+    __device__ __forceinline__ void stage_b(int n, const GasConst& gc, Sink& sink) {
+        if (PH >= 3) {
+            float gr2[NCOMP], gl2[NCOMP];
+            cell_split_flux(uhl, gc, gr2, gl2);                             // (d), cell m
+            if (PH >= 4) {                                                  // m >= 2
                 float ar0[NCOMP], al0[NCOMP];
 #pragma unroll
                 for (int k = 0; k < NCOMP; ++k) {
-                    ar0[k] = gr2[k] - gr2_prev[k];                          // G^R_m - G^R_{m-1}
-                    al0[k] = gl2[k] - gl2_prev[k];                          // G^L_m - G^L_{m-1}
+                    ar0[k] = gr2[k] - gr2_prev[k];
+                    al0[k] = gl2[k] - gl2_prev[k];
                 }
                 float xr[NCOMP];
-                if (PH >= 4) {                                              // m >= 3: (e) right-moving, (m-1|m)
+                if (PH >= 5) {                                              // m >= 3: (e) right-moving, (m-1|m)
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) xr[k] = limited<+1>(gr2_prev[k], ar1[k], ar0[k]);
                 }
-                if (PH >= 5) {                                              // m >= 4: (e) left-moving, (m-2|m-1)
+                if (PH >= 6) {                                              // m >= 4: (e) left-moving, (m-2|m-1)
                     float fh[NCOMP];
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) {
-                        // a = G^L_{m-1}-G^L_m = -al0, b = G^L_{m-2}-G^L_{m-1} = -al1: a b = al0 al1, a+b = -(al0+al1)
                         const float xl = limited<-1>(gl2_prev[k], al0[k], al1[k]);
                         fh[k] = xr_prev[k] - xl;
                     }
                     if (WANT_FACE) {
-                        const int i = n - 3;                                // interface (i | i+1), i = m-2
+                        const int i = n - 4;                                // interface (i | i+1), i = m-2
                         if (i == NG - 1 || i == NG + PS / 2 - 1 || i == NG + PS - 1) {
                             float ff[NCOMP];
 #pragma unroll
@@ -186,18 +191,18 @@ struct RowMarch {
                             sink.face(i == NG - 1 ? 0 : (i == NG + PS - 1 ? 2 : 1), ff);
                         }
                     }
-                    if (PH >= 6) {                                          // m >= 5: (f) cell j = m-2 = n-3
+                    if (PH >= 7) {                                          // m >= 5: (f) cell j = m-2 = n-4
                         float un[NCOMP];
 #pragma unroll
-                        for (int k = 0; k < NCOMP; ++k) un[k] = fmaf(-gc.kh, fh[k] - fh_prev[k], u3[k]);
-                        sink.template cell<ODD>(n - 3, un);
+                        for (int k = 0; k < NCOMP; ++k) un[k] = fmaf(-gc.kh, fh[k] - fh_prev[k], u4[k]);
+                        sink.template cell<ODD>(n - 4, un);
                     }
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) fh_prev[k] = fh[k];
                 }
 #pragma unroll
                 for (int k = 0; k < NCOMP; ++k) {
-                    if (PH >= 4) xr_prev[k] = xr[k];
+                    if (PH >= 5) xr_prev[k] = xr[k];
                     ar1[k] = ar0[k];
                     al1[k] = al0[k];
                 }
@@ -208,8 +213,24 @@ struct RowMarch {
                 gl2_prev[k] = gl2[k];
             }
         }
+    }
+
+    // stage A of step n: coefficients of cell n (a), midpoint state of cell n-1 (b)+(c) into the latch; window shift
+    template <int PH>
+    __device__ __forceinline__ void stage_a(const float (&u)[NCOMP], const GasConst& gc) {
+        const HalfCoef h = half_coef(u, gc);
+        if (PH >= 2) {
+            const float dP = __fsub_rn(P2, h.P), dPv = __fsub_rn(Pv2, h.Pv);
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) {
+                float b = (k == 1) ? fmaf(sig1, u1[k], dP) : ((k == 4) ? fmaf(sig1, u1[k], dPv) : __fmul_rn(sig1, u1[k]));
+                b = fmaf(cp2, u2[k], b);
+                uhl[k] = fmaf(h.cm, u[k], b);
+            }
+        }
 #pragma unroll
         for (int k = 0; k < NCOMP; ++k) {
+            if (PH >= 3) u4[k] = u3[k];
             if (PH >= 2) u3[k] = u2[k];
             if (PH >= 1) u2[k] = u1[k];
             u1[k] = u[k];
@@ -218,17 +239,16 @@ struct RowMarch {
         cp1 = h.cp; P1 = h.P; Pv1 = h.Pv; sig1 = h.sig;
     }
 
-    // Cells are fetched two at a time (n even, n+1) by `load(n, ua, ub)`: a row along x is read with 64-bit
-    // shared-memory loads.  gate.acquire(n) is called before cells n, n+1 are read and gate.release(n) once they are in
-    // registers (the march never reads them again): the pipelined kernel uses this to wait for / hand back z-planes.
     template <int PH0, int PH1, class Src, class Gate>
     __device__ __forceinline__ void pair(Src& src, int n, const GasConst& gc, Sink& sink, Gate& gate) {
         float ua[NCOMP], ub[NCOMP];
         gate.acquire(n);
         src.load(n, ua, ub);
         gate.release(n);
-        step<PH0, 1>(ua, n, gc, sink);          // n is even: j = n-3 is odd
-        step<PH1, 0>(ub, n + 1, gc, sink);
+        stage_b<PH0, 0>(n, gc, sink);           // n is even: j = n-4 is even
+        stage_a<PH0>(ua, gc);
+        stage_b<PH1, 1>(n + 1, gc, sink);
+        stage_a<PH1>(ub, gc);
     }
 
     template <class Src, class Gate>
@@ -236,8 +256,10 @@ struct RowMarch {
         pair<0, 1>(src, 0, gc, sink, gate);
         pair<2, 3>(src, 2, gc, sink, gate);
         pair<4, 5>(src, 4, gc, sink, gate);
+        pair<6, 7>(src, 6, gc, sink, gate);
 #pragma unroll MARCH_UNROLL
-        for (int n = 6; n < NP; n += 2) pair<6, 6>(src, n, gc, sink, gate);
+        for (int n = 8; n < NP; n += 2) pair<7, 7>(src, n, gc, sink, gate);
+        stage_b<7, 0>(NP, gc, sink);            // drain: cell j = 18
     }
 };
 
