@@ -320,6 +320,26 @@ def run_ours(args):
         except Exception as ex:      # e.g. not enough pinnable host memory
             e2e = dict(value=None, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0, error=str(ex)[:200])
 
+    # NEXT-3 (reported separately, not part of the step): device-side ghost fill of the same batch seen as a periodic
+    # box of groups — reads every interior once, writes every padded group once.  It overwrites d_in, so it runs last.
+    ghost_fill = None
+    if rank == 0 and not args.no_ghost_fill:
+        gxyz = round(n ** (1.0 / 3.0))
+        box = (gxyz, gxyz, gxyz) if gxyz ** 3 == n else (n, 1, 1)
+        for _ in range(2):
+            hydro.gamer_hydro_ghost_fill(d_out, d_in, box[0], box[1], box[2], stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(5):
+            hydro.gamer_hydro_ghost_fill(d_out, d_in, box[0], box[1], box[2], stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        gf_ms = e0.elapsed_time(e1) / 5
+        gf_gbs = n * BYTES_PER_GROUP / (gf_ms * 1e-3) / 1e9
+        ghost_fill = dict(api="gamer_hydro_ghost_fill", box_groups=list(box), ms=gf_ms, bound="hbm", achieved=gf_gbs,
+                          peak=peaks["hbm_gbs"], unit="GB/s", frac=gf_gbs / peaks["hbm_gbs"],
+                          algorithmic_bytes=n * BYTES_PER_GROUP)
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cores = os.cpu_count() or 1
@@ -334,6 +354,7 @@ def run_ours(args):
                                 launch=info),
                     roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
                     cpu_baseline=cpu_baseline, e2e=e2e, gpu_launches=args.steps, clocks=clocks,
+                    next3_ghost_fill=ghost_fill,
                     parity_spot_check_max_rel=parity)
         print(json.dumps(line))
     if dist is not None:
@@ -355,6 +376,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
     ap.add_argument("--no-check", action="store_true")
+    ap.add_argument("--no-ghost-fill", action="store_true", help="skip the separate ghost-fill measurement")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

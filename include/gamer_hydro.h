@@ -21,8 +21,9 @@
  *                        denominator of the CFL condition Eq.30 (:418-426: "a single floating-point value per patch
  *                        group").
  *
- * WHAT THE LIBRARY DOES NOT DO: it does not fill ghost zones (the caller's "preparation step", :322), it does not
- * choose dt (:418-426 — it only offers the per-group reduction), it applies no density or pressure floor (the
+ * WHAT gamer_hydro_advance* DO NOT DO: they do not fill ghost zones (the caller's "preparation step", :322 — see
+ * gamer_hydro_ghost_fill for the single-level case), they do not choose dt (:418-426 — they only offer the per-group
+ * reduction; gamer_hydro_run_uniform does), and nothing applies a density or pressure floor (the
  * paper names none): non-physical input (rho <= 0 or P <= 0) yields NaN/Inf in the affected cells, silently.
  *
  * OWNERSHIP: the caller owns every buffer.  `d_*` are DEVICE pointers (cudaMalloc or equivalent) valid on the
@@ -89,6 +90,28 @@ GAMER_API size_t gamer_hydro_face_flux_floats(long long n_groups);
 GAMER_API int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups, int ghost,
                              float dt, float dh, float gamma, int backward,
                              long long groups_per_chunk, int n_streams);
+
+/* NEXT-3 — device-side preparation step for a SINGLE-LEVEL tiling ("ghost zones ... filled by directly
+ * copying from the sibling patches"; :430-432, :647 name this CPU step the bottleneck of the code).  gx*gy*gz groups tile
+ * a box of 16gx x 16gy x 16gz cells, group index g = (kz*gy + ky)*gx + kx.  d_interior: [g][v][16][16][16] (the layout
+ * of d_out), read only.  d_padded: [g][v][22][22][22] (the layout of d_in); every interior cell is written from the
+ * group's own interior and every ghost cell from the interior of the neighbouring group.  bc_x, bc_y, bc_z per axis:
+ * 0 = periodic box; 1 = "keep": ghost cells that lie beyond that end of the box are NOT written, they keep what the
+ * caller put there (a Dirichlet boundary).  Pure data movement, bit exact.  Asynchronous on `stream`.
+ * gx, gy, gz < 1, a flag other than 0/1, a NULL or misaligned pointer -> GAMER_EINVAL. */
+GAMER_API int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int gy, int gz,
+                           int bc_x, int bc_y, int bc_z, void* stream);
+
+/* NEXT-3 — multi-step driver on such a box, entirely on the device (no host round trip between steps).  Each of the
+ * n_steps steps does: dt = cfl * dh / max over ALL padded cells of (c_s + max_i |v_i|) (Eq.30, PAPER.md:418-426;
+ * fp32, reading R10); one forward pass gamer_hydro_advance(d_padded -> d_interior) with that dt (read from
+ * device memory, constants formed exactly as on the host); gamer_hydro_ghost_fill(d_interior -> d_padded).  On return
+ * (asynchronous on `stream`) d_padded holds the ghost-filled state after n_steps and d_interior its interiors.
+ * d_work: >= 4 floats of device scratch, 16-byte aligned.  d_dt_log: optional device array of n_steps floats that
+ * receives the dt of every step (NULL = off). */
+GAMER_API int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, int gz,
+                            int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dh, float gamma,
+                            float* d_work, float* d_dt_log, void* stream);
 
 /* Launch geometry the library will use on the current device, for reporting: any pointer may be NULL.
  * grid = number of persistent CTAs for n_groups, block = threads per CTA, smem = dynamic shared memory per CTA in

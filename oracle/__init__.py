@@ -132,3 +132,64 @@ def count_ops():
 
 def has_openmp():
     return bool(lib().oracle_has_openmp())
+
+
+def ghost_fill(interior, grid, bc=(0, 0, 0), padded=None):
+    """Preparation step on a single-level tiling, written out cell by cell (ghost zones of a patch group
+    are copied from the sibling patches).  Pure data movement.
+
+    interior: [G][5][16][16][16], G = gz*gy*gx groups tiling a box, grid = (gz, gy, gx), g = (kz*gy + ky)*gx + kx.
+    bc = (bc_x, bc_y, bc_z): 0 periodic; 1 = ghost cells beyond that end of the box keep the value they have in
+    `padded` (required then).  Returns [G][5][22][22][22].
+    """
+    a = np.asarray(interior)
+    gz, gy, gx = grid
+    assert a.shape == (gz * gy * gx, NCOMP, PS, PS, PS), a.shape
+    out = np.array(padded, dtype=a.dtype, copy=True) if padded is not None else np.full(
+        (a.shape[0], NCOMP, NP, NP, NP), np.nan, a.dtype)
+    n = (gx * PS, gy * PS, gz * PS)
+    for kz in range(gz):
+        for ky in range(gy):
+            for kx in range(gx):
+                g = (kz * gy + ky) * gx + kx
+                k = (kx, ky, kz)
+                # per axis: source group coordinate and source interior index of each of the 22 padded positions
+                src_grp, src_idx, ok = [], [], []
+                for ax in range(3):
+                    c = k[ax] * PS + np.arange(NP) - NGHOST          # cell coordinate in the box
+                    inside = (c >= 0) & (c < n[ax])
+                    c = np.mod(c, n[ax])
+                    src_grp.append(c // PS)
+                    src_idx.append(c % PS)
+                    ok.append(inside | (bc[ax] == 0))
+                # all 22^3 padded positions of this group at once (index arrays instead of three nested loops)
+                Z, Y, X = np.meshgrid(np.arange(NP), np.arange(NP), np.arange(NP), indexing="ij")
+                sg = (src_grp[2][Z] * gy + src_grp[1][Y]) * gx + src_grp[0][X]
+                write = ok[2][Z] & ok[1][Y] & ok[0][X]
+                vals = a[sg, :, src_idx[2][Z], src_idx[1][Y], src_idx[0][X]]        # [22][22][22][5]
+                out[g][:, write] = vals[write].T
+    return out
+
+
+def max_signal_speed(padded, gamma):
+    """max over all cells of c_s + max_i |v_i| (Eq.30), in the array's own precision."""
+    u = np.asarray(padded)
+    t = u.dtype.type
+    rho = u[:, 0]
+    v = np.abs(u[:, 1:4]) / rho[:, None]
+    p = (t(gamma) - t(1)) * (u[:, 4] - t(0.5) * (u[:, 1] ** 2 + u[:, 2] ** 2 + u[:, 3] ** 2) / rho)
+    return (np.sqrt(t(gamma) * p / rho) + v.max(axis=1)).max()
+
+
+def run_uniform(padded, grid, bc, n_steps, cfl, dh, gamma, n_threads=1):
+    """n_steps of {dt from Eq.30 over all padded cells; one forward pass; ghost refill} (DESIGN.md NEXT-3).
+    Returns (padded state, list of dt)."""
+    u = np.array(padded, copy=True)
+    t = u.dtype.type
+    dts = []
+    for _ in range(n_steps):
+        dt = t(cfl) * t(dh) / max_signal_speed(u, gamma)
+        out = hydro_advance(u, dt, dh, gamma, n_threads=n_threads)
+        u = ghost_fill(out, grid, bc, padded=u)
+        dts.append(float(dt))
+    return u, dts

@@ -11,6 +11,7 @@
 
 #include "../../include/gamer_hydro.h"
 #include "hydro_kernel.cuh"
+#include "uniform_grid.cuh"
 
 namespace {
 
@@ -26,7 +27,7 @@ int fail(int code, const char* fmt, ...) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-using KernelFn = void (*)(const float*, float*, long long, gamer::GasConst, float*, float*);
+using KernelFn = void (*)(const float*, float*, long long, gamer::GasConst, float*, float*, const float*);
 
 KernelFn pick_kernel(bool backward, bool face, bool speed) {
     using namespace gamer;
@@ -104,8 +105,10 @@ gamer::GasConst make_const(float dt, float dh, float gamma) {
     gc.ggm1 = gamma * (gamma - 1.0f);
     gc.kq = 0.25f * k;
     gc.kh = 0.5f * k;
+    gc.dh = dh;
+    gc.sg = sqrtf(gc.ggm1);
     gc.kq_gm1 = gc.kq * gc.gm1;
-    gc.kq_sg = gc.kq * sqrtf(gc.ggm1);
+    gc.kq_sg = gc.kq * gc.sg;
     return gc;
 }
 
@@ -118,7 +121,7 @@ int launch(const float* d_in, float* d_out, long long n_groups, float dt, float 
     if (rc != GAMER_OK) return rc;
     const int grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
     fn<<<grid, gamer::BLOCK_THREADS, gamer::SMEM_BYTES, stream>>>(d_in, d_out, n_groups, make_const(dt, dh, gamma),
-                                                                  d_face, d_speed);
+                                                                  d_face, d_speed, nullptr);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
     return GAMER_OK;
@@ -210,6 +213,63 @@ int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups
         if (streams[s]) cudaStreamDestroy(streams[s]);
     }
     return status;
+}
+
+static int check_box(int gx, int gy, int gz, int bc_x, int bc_y, int bc_z) {
+    if (gx < 1 || gy < 1 || gz < 1) return fail(GAMER_EINVAL, "box of %d x %d x %d groups", gx, gy, gz);
+    if ((long long)gx * gy * gz > (1ll << 31) / gamer::NCOMP - 1) return fail(GAMER_EINVAL, "too many groups for one launch");
+    if ((bc_x | bc_y | bc_z) & ~1) return fail(GAMER_EINVAL, "boundary flags must be 0 (periodic) or 1 (keep)");
+    return GAMER_OK;
+}
+
+int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int gy, int gz, int bc_x, int bc_y,
+                           int bc_z, void* stream) {
+    int rc = check_box(gx, gy, gz, bc_x, bc_y, bc_z);
+    if (rc != GAMER_OK) return rc;
+    if (d_interior == nullptr || d_padded == nullptr) return fail(GAMER_EINVAL, "NULL pointer");
+    if (!aligned16(d_interior) || !aligned16(d_padded)) return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
+    g_err[0] = '\0';
+    const long long n = (long long)gx * gy * gz;
+    gamer::BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
+    gamer::ghost_fill_kernel<<<(unsigned int)(n * gamer::NCOMP), gamer::GF_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
+        d_interior, d_padded, geo);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(GAMER_ECUDA, "ghost_fill launch: %s", cudaGetErrorString(e));
+    return GAMER_OK;
+}
+
+int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, int gz, int bc_x, int bc_y, int bc_z,
+                            int n_steps, float cfl, float dh, float gamma, float* d_work, float* d_dt_log,
+                            void* stream_) {
+    int rc = check_box(gx, gy, gz, bc_x, bc_y, bc_z);
+    if (rc != GAMER_OK) return rc;
+    const long long n = (long long)gx * gy * gz;
+    rc = validate(d_padded, d_interior, n, gamer::NG, 0.f, dh, gamma, 0, d_work, d_dt_log);
+    if (rc != GAMER_OK) return rc;
+    if (d_work == nullptr) return fail(GAMER_EINVAL, "d_work must point to at least 4 floats of device memory");
+    if (n_steps < 0 || !(cfl > 0.f)) return fail(GAMER_EINVAL, "n_steps must be >= 0 and cfl > 0");
+    g_err[0] = '\0';
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    using namespace gamer;
+    KernelFn fn = hydro_advance_kernel<false, false, false, true>;
+    int sm_count = 0;
+    rc = prepare(reinterpret_cast<const void*>(fn), 8, SMEM_BYTES, &sm_count);
+    if (rc != GAMER_OK) return rc;
+    const int grid = (int)(n < (long long)sm_count ? n : (long long)sm_count);
+    const int red_grid = (int)(n < 4ll * sm_count ? n : 4ll * sm_count);
+    BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
+    cudaError_t e = cudaMemsetAsync(d_work, 0, 4 * sizeof(float), stream);
+    for (int s = 0; s < n_steps && e == cudaSuccess; ++s) {
+        // Eq.30 on the current padded state -> dt in d_work[1]; one forward pass with that dt; ghost refill
+        max_speed_kernel<<<red_grid, 256, 0, stream>>>(d_padded, n, gamma, reinterpret_cast<unsigned int*>(d_work));
+        cfl_dt_kernel<<<1, 1, 0, stream>>>(d_work, cfl, dh, d_dt_log ? d_dt_log + s : nullptr);
+        fn<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, make_const(0.f, dh, gamma), nullptr,
+                                                        nullptr, d_work + 1);
+        ghost_fill_kernel<<<(unsigned int)(n * NCOMP), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) return fail(GAMER_ECUDA, "run_uniform: %s", cudaGetErrorString(e));
+    return GAMER_OK;
 }
 
 int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread) {

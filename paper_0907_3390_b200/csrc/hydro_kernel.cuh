@@ -363,10 +363,21 @@ __device__ __forceinline__ void reduce_speed(Ctl* ctl, float speed, unsigned int
     }
 }
 
-template <bool BACKWARD, bool WANT_FACE, bool WANT_SPEED>
+// DEVICE_DT: the time step is read from *d_dt (written by an earlier kernel on the same stream, e.g. cfl_dt_kernel)
+// and the dt-dependent constants are formed here exactly as make_const() forms them on the host.
+template <bool BACKWARD, bool WANT_FACE, bool WANT_SPEED, bool DEVICE_DT = false>
 __global__ void __launch_bounds__(BLOCK_THREADS, 1)
-hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long long n_groups, GasConst gc,
-                     float* __restrict__ face_flux, float* __restrict__ group_maxspeed) {
+hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long long n_groups, GasConst gc_in,
+                     float* __restrict__ face_flux, float* __restrict__ group_maxspeed,
+                     const float* __restrict__ d_dt = nullptr) {
+    GasConst gc = gc_in;
+    if (DEVICE_DT) {
+        const float k = __fdiv_rn(*d_dt, gc.dh);
+        gc.kq = __fmul_rn(0.25f, k);
+        gc.kh = __fmul_rn(0.5f, k);
+        gc.kq_gm1 = __fmul_rn(gc.kq, gc.gm1);
+        gc.kq_sg = __fmul_rn(gc.kq, gc.sg);
+    }
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* smem = reinterpret_cast<float*>(smem_raw);
     Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + GROUP_IN_BYTES);

@@ -37,6 +37,8 @@ struct GasConst {
     float kh;       // (dt/dh) / 2
     float kq_gm1;   // kq (gamma - 1)
     float kq_sg;    // kq sqrt(gamma (gamma - 1))
+    float dh;       // cell size            } only read when the time step comes from device memory
+    float sg;       // sqrt(gamma (gamma-1)) }
 };
 
 __device__ __forceinline__ float rcp_fast(float x) {

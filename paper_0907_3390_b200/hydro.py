@@ -45,6 +45,10 @@ def lib():
         L.gamer_hydro_face_flux_floats.argtypes = [ll]
         L.gamer_hydro_pipeline_run.restype = ci
         L.gamer_hydro_pipeline_run.argtypes = [vp, vp, ll, ci, cf, cf, cf, ci, ll, ci]
+        L.gamer_hydro_ghost_fill.restype = ci
+        L.gamer_hydro_ghost_fill.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, vp]
+        L.gamer_hydro_run_uniform.restype = ci
+        L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
         L.gamer_hydro_launch_info.restype = ci
         L.gamer_hydro_launch_info.argtypes = [ll] + [ctypes.POINTER(ci)] * 4
         L.gamer_last_error.restype = ctypes.c_char_p
@@ -124,6 +128,25 @@ def gamer_hydro_pipeline_run(h_in, h_out, n_groups, ghost, dt, dh, gamma, backwa
     """Host buffers in, host buffers out (pinned for overlap), synchronous (Fig.5)."""
     rc = lib().gamer_hydro_pipeline_run(_ptr(h_in), _ptr(h_out), n_groups, ghost, dt, dh, gamma, int(backward),
                                         groups_per_chunk, n_streams)
+    if check:
+        _check(rc)
+    return rc
+
+
+def gamer_hydro_ghost_fill(d_interior, d_padded, gx, gy, gz, bc_x=0, bc_y=0, bc_z=0, stream=None, check=True):
+    """Device-side ghost fill of a single-level tiling of gx*gy*gz groups.  bc: 0 periodic, 1 keep."""
+    rc = lib().gamer_hydro_ghost_fill(_ptr(d_interior), _ptr(d_padded), gx, gy, gz, bc_x, bc_y, bc_z,
+                                      _stream_ptr(stream))
+    if check:
+        _check(rc)
+    return rc
+
+
+def gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, n_steps, cfl, dh, gamma, d_work,
+                            d_dt_log=None, stream=None, check=True):
+    """n_steps of {CFL dt on the device, forward pass, ghost fill} without leaving the device."""
+    rc = lib().gamer_hydro_run_uniform(_ptr(d_padded), _ptr(d_interior), gx, gy, gz, bc_x, bc_y, bc_z, n_steps, cfl, dh,
+                                       gamma, _ptr(d_work), _ptr(d_dt_log), _stream_ptr(stream))
     if check:
         _check(rc)
     return rc

@@ -1,0 +1,143 @@
+"""NEXT-3: device-side ghost fill of a single-level tiling and the multi-step driver.
+
+CPU part: the oracle's cell-by-cell ghost fill is pinned against an independent construction (np.pad of
+the assembled box, workloads.box_to_groups) and against hand-picked cells.  GPU part (-m gpu): the CUDA ghost fill is
+bit-exact against the oracle; gamer_hydro_run_uniform reproduces config 2 (Sod, 100 steps) without host round trips."""
+import numpy as np
+import pytest
+
+import oracle
+import riemann_exact
+from paper_0907_3390_b200 import hydro
+from paper_0907_3390_b200 import workloads as W
+
+
+def random_interiors(grid, seed=7):
+    gz, gy, gx = grid
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((gz * gy * gx, 5, 16, 16, 16)).astype(np.float32)
+
+
+@pytest.mark.parametrize("grid", [(1, 1, 1), (2, 1, 3), (2, 3, 2)])
+def test_oracle_ghost_fill_periodic_equals_padded_box(grid):
+    a = random_interiors(grid)
+    ref = W.box_to_groups(W.groups_to_box(a, grid))          # np.pad(mode="wrap") of the assembled box, then cut
+    got = oracle.ghost_fill(a, grid)
+    assert got.dtype == a.dtype and np.array_equal(got, ref)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_oracle_ghost_fill_keep_is_dirichlet(axis):
+    grid = (2, 2, 2)
+    a = random_interiors(grid, 11)
+    lo = np.arange(1, 6, dtype=np.float32)
+    hi = -np.arange(1, 6, dtype=np.float32)
+    ref = W.box_to_groups(W.groups_to_box(a, grid), dirichlet_axis=axis, lo_state=lo, hi_state=hi)
+    bc = [0, 0, 0]
+    bc[axis] = 1
+    # the caller's padded array holds the boundary states in the ghost cells beyond the box (anything elsewhere)
+    pre = np.full_like(ref, 123.0)
+    sl = [slice(None)] * 5
+    sl[4 - axis] = slice(0, 3)
+    pre[tuple(sl)] = lo.reshape(1, 5, 1, 1, 1)
+    sl[4 - axis] = slice(19, 22)
+    pre[tuple(sl)] = hi.reshape(1, 5, 1, 1, 1)
+    got = oracle.ghost_fill(a, grid, tuple(bc), padded=pre)
+    # interior groups' inner faces are neighbours' data; only the box ends keep the states
+    assert np.array_equal(got, ref)
+
+
+def test_oracle_ghost_fill_hand_picked_cells():
+    grid = (1, 2, 3)                                          # gz, gy, gx
+    a = random_interiors(grid, 3)
+    p = oracle.ghost_fill(a, grid)
+    g = lambda kz, ky, kx: (kz * 2 + ky) * 3 + kx
+    # padded (z,y,x) = (3,3,0) of group (0,0,0): box cell x = -3 -> wraps to group kx=2, interior x = 13
+    assert np.array_equal(p[g(0, 0, 0), :, 3, 3, 0], a[g(0, 0, 2), :, 0, 0, 13])
+    # padded x = 21 of group kx=1: box cell x = 16+18 = 34 -> group kx=2, interior x = 2
+    assert np.array_equal(p[g(0, 1, 1), :, 5, 4, 21], a[g(0, 1, 2), :, 2, 1, 2])
+    # padded y = 1 of group ky=0: box cell y = -2 -> ky=1, interior y = 14; z ghost wraps onto the same group (gz = 1)
+    assert np.array_equal(p[g(0, 0, 1), :, 0, 1, 10], a[g(0, 1, 1), :, 13, 14, 7])
+    # interior is the group's own
+    assert np.array_equal(p[:, :, 3:19, 3:19, 3:19], a)
+
+
+def test_oracle_run_uniform_is_the_written_out_loop():
+    c = W.config1()
+    grid = (2, 2, 2)
+    u = c["inp"].astype(np.float64)
+    got, dts = oracle.run_uniform(u, grid, (0, 0, 0), 2, 0.5, c["dh"], c["gamma"])
+    v = u.copy()
+    for s in range(2):
+        dt = 0.5 * c["dh"] / W.max_signal_speed(v, c["gamma"])        # workloads' own fp64 Eq.30
+        assert abs(dt - dts[s]) <= 1e-13 * dt
+        out = oracle.hydro_advance(v, dts[s], c["dh"], c["gamma"])
+        v = W.box_to_groups(W.groups_to_box(out, grid))
+    assert np.array_equal(got, v)
+
+
+def test_ghost_fill_argument_validation_needs_no_device():
+    import ctypes
+    L = hydro.lib()
+    buf = (ctypes.c_float * 64)()
+    a16 = (ctypes.addressof(buf) + 15) & ~15
+    assert L.gamer_hydro_ghost_fill(a16, a16, 0, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_ghost_fill(a16, a16, 1, 1, 1, 2, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_ghost_fill(None, a16, 1, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_ghost_fill(a16, a16 + 4, 1, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_run_uniform(a16, a16, 1, 1, 1, 0, 0, 0, 1, 0.5, 1.0, 1.4, None, None, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_run_uniform(a16, a16, 1, 1, 1, 0, 0, 0, 1, 0.0, 1.0, 1.4, a16, None, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_run_uniform(a16, a16, 1, 1, 1, 0, 0, 0, -1, 0.5, 1.0, 1.4, a16, None, None) == hydro.GAMER_EINVAL
+
+
+# ---------------------------------------------------------------------------------------------------------- GPU
+@pytest.mark.gpu
+@pytest.mark.parametrize("grid,bc", [((1, 1, 1), (0, 0, 0)), ((2, 3, 2), (0, 0, 0)), ((2, 2, 3), (1, 0, 0)),
+                                     ((3, 2, 2), (0, 1, 1)), ((2, 2, 2), (1, 1, 1))])
+def test_gpu_ghost_fill_bit_exact(grid, bc):
+    import torch
+    gz, gy, gx = grid
+    a = random_interiors(grid, 5)
+    pre = np.random.default_rng(9).standard_normal((a.shape[0], 5, 22, 22, 22)).astype(np.float32)
+    ref = oracle.ghost_fill(a, grid, bc, padded=pre)
+    d_a = torch.from_numpy(a).cuda()
+    d_p = torch.from_numpy(pre).cuda()
+    hydro.gamer_hydro_ghost_fill(d_a, d_p, gx, gy, gz, *bc)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_p.cpu().numpy(), ref)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_gpu_run_uniform_config2_sod(axis):
+    """Config 2 on the device only: 100 steps of {Eq.30, forward pass, ghost fill} in one call.  Compared with the
+    oracle's chain (same loop, fp32, <= 1e-3 as in DESIGN.md R16), with its dt sequence, and with the exact solution."""
+    import torch
+    gamma, dh, nsteps = 1.4, 1.0 / 128, 100
+    U, left, right = W.config2_box(axis, gamma)
+    grid = tuple(s // 16 for s in U.shape[1:])
+    gz, gy, gx = grid
+    l32, r32 = left.astype(np.float32), right.astype(np.float32)
+    inp = W.box_to_groups(U.astype(np.float32), dirichlet_axis=axis, lo_state=l32, hi_state=r32)
+    bc = [0, 0, 0]
+    bc[axis] = 1
+    d_p = torch.from_numpy(inp).cuda()
+    d_i = torch.empty((inp.shape[0], 5, 16, 16, 16), dtype=torch.float32, device="cuda")
+    d_work = torch.zeros(4, dtype=torch.float32, device="cuda")
+    d_log = torch.zeros(nsteps, dtype=torch.float32, device="cuda")
+    hydro.gamer_hydro_run_uniform(d_p, d_i, gx, gy, gz, bc[0], bc[1], bc[2], nsteps, 0.5, dh, gamma, d_work, d_log)
+    torch.cuda.synchronize()
+    got, dts = d_p.cpu().numpy(), d_log.cpu().numpy().astype(np.float64)
+    # the transverse sweeps are exact no-ops, so the oracle chain can run on one column of groups
+    ref, ref_dts = oracle.run_uniform(inp, grid, tuple(bc), nsteps, 0.5, dh, gamma, n_threads=8)
+    assert np.max(np.abs(dts - np.array(ref_dts)) / np.array(ref_dts)) <= 2e-6
+    e = W.parity_error(got[:, :, 3:19, 3:19, 3:19], ref[:, :, 3:19, 3:19, 3:19], gamma)
+    assert e["max_rel"] <= 1e-3, e
+    assert np.array_equal(got[:, :, 3:19, 3:19, 3:19], d_i.cpu().numpy())
+    box = W.groups_to_box(got[:, :, 3:19, 3:19, 3:19], grid)
+    sel = [0, 0, 0]
+    sel[2 - axis] = slice(None)
+    rho = box[(0,) + tuple(sel)].astype(np.float64)
+    x = (np.arange(128) + 0.5) * dh
+    rho_e, _, _ = riemann_exact.sample((x - 0.5) / dts.sum(), 1, 0, 1, 0.125, 0, 0.1, gamma)
+    assert np.mean(np.abs(rho - rho_e)) <= 1.0e-2
