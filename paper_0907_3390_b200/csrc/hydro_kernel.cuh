@@ -145,13 +145,13 @@ struct FinalSink {
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) dst[k][j * STRIDE] = u[k];
         }
-        if (WANT_SPEED) {    // Eq.30 on the updated cell
-            const float rinv = 1.0f / u[0];
+        if (WANT_SPEED) {    // Eq.30 on the updated cell; approximate reciprocal / root (1-2 ulp)
+            const float rinv = rcp_fast(u[0]);
             float q = u[2] * u[2];
             q = fmaf(u[3], u[3], q);
             q = fmaf(u[1], u[1], q);
             const float eint = fmaf(-q, 0.5f * rinv, u[4]);
-            const float cs = sqrtf((ggm1 * eint) * rinv);
+            const float cs = sqrt_fast((ggm1 * eint) * rinv);
             const float vm = fmaxf(fmaxf(fabsf(u[1]), fabsf(u[2])), fabsf(u[3])) * rinv;
             speed = fmaxf(speed, cs + vm);
         }
@@ -326,6 +326,16 @@ struct ZPlaneGate {
     }
 };
 
+// Gate of the backward z march (the first sweep): wait for a load chunk when the march reaches its first plane.
+struct ChunkWaitGate {
+    Ctl* ctl;
+    uint32_t parity;
+    __device__ __forceinline__ void acquire(int n) {
+        if (n % (2 * CHUNK_PAIRS) == 0) mbar_wait_poll(&ctl->full[n / (2 * CHUNK_PAIRS)], parity);
+    }
+    __device__ __forceinline__ void release(int) {}
+};
+
 // The loader warp, during the z sweep of a group that has a successor.
 __device__ __forceinline__ void load_next_group(float* smem, Ctl* ctl, const float* __restrict__ in_next) {
 #pragma unroll
@@ -448,17 +458,20 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             // no CTA-wide barrier: a plane is overwritten only after all z threads have read it (BAR_ZFREE), and the
             // next group's x tasks wait for their planes (BAR_FULL)
         } else {
-            uint64_t* bar = &ctl->full[0];
+            // The group arrives in the same three chunks of z-planes; the z march (first sweep) waits for a chunk only
+            // when it reaches its first plane, so all but the first chunk land under the march.
             if (threadIdx.x == 0) {
                 fence_proxy_async();  // generic-proxy accesses of the previous group are ordered before the async write
-                mbar_expect_tx(bar, GROUP_IN_BYTES);
-                bulk_g2s(smem, in + g * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES, bar);
+                const float* in_g = in + g * (long long)GROUP_IN_FLOATS;
+                for (int c = 0; c < N_CHUNK; ++c) load_chunk(smem, ctl, in_g, c);
                 const long long gn = g + gridDim.x;
                 if (gn < n_groups) bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES);
             }
-            mbar_wait_poll(bar, parity);
+            ChunkWaitGate zgate;
+            zgate.ctl = ctl;
+            zgate.parity = parity;
             PHASE_ACC(0);
-            sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
+            sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, zgate);
             __syncthreads();
             PHASE_ACC(1);
             sweep<1, 0, NP, NG, PS, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
