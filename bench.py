@@ -371,8 +371,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[3, 4, 5])
     ap.add_argument("--groups", type=int, default=None, help="debug: override the number of groups")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--chunk", type=int, default=2048, help="pipeline: groups per chunk (N_g)")
-    ap.add_argument("--streams", type=int, default=4, help="pipeline: number of streams (N_s)")
+    ap.add_argument("--chunk", type=int, default=512, help="pipeline: groups per chunk (N_g)")
+    ap.add_argument("--streams", type=int, default=3, help="pipeline: number of streams (N_s)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
     ap.add_argument("--no-check", action="store_true")
