@@ -320,6 +320,25 @@ def run_ours(args):
         except Exception as ex:      # e.g. not enough pinnable host memory
             e2e = dict(value=None, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0, error=str(ex)[:200])
 
+    # NEXT-1/2 (reported separately): the same forward pass with the optional outputs switched on
+    optional_outputs = None
+    if rank == 0 and not args.no_ghost_fill:
+        d_face = torch.empty((n, 3, 3, 5, 16, 16), dtype=torch.float32, device=device)
+        d_speed = torch.empty((n,), dtype=torch.float32, device=device)
+        optional_outputs = {}
+        for name, kw in (("maxspeed", dict(d_group_maxspeed=d_speed)),
+                         ("face_flux+maxspeed", dict(d_face_flux=d_face, d_group_maxspeed=d_speed))):
+            for _ in range(2):
+                hydro.gamer_hydro_advance_ex(d_in, d_out, n, 3, dt, dh, gamma, 0, stream=stream, **kw)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(5):
+                hydro.gamer_hydro_advance_ex(d_in, d_out, n, 3, dt, dh, gamma, 0, stream=stream, **kw)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            optional_outputs[name] = dict(ns_per_group=e0.elapsed_time(e1) / 5 * 1e6 / n)
+        del d_face, d_speed
+
     # NEXT-3 (reported separately, not part of the step): device-side ghost fill of the same batch seen as a periodic
     # box of groups — reads every interior once, writes every padded group once.  It overwrites d_in, so it runs last.
     ghost_fill = None
@@ -354,7 +373,7 @@ def run_ours(args):
                                 launch=info),
                     roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
                     cpu_baseline=cpu_baseline, e2e=e2e, gpu_launches=args.steps, clocks=clocks,
-                    next3_ghost_fill=ghost_fill,
+                    next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs,
                     parity_spot_check_max_rel=parity)
         print(json.dumps(line))
     if dist is not None:
