@@ -217,7 +217,7 @@ int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups
 
 static int check_box(int gx, int gy, int gz, int bc_x, int bc_y, int bc_z) {
     if (gx < 1 || gy < 1 || gz < 1) return fail(GAMER_EINVAL, "box of %d x %d x %d groups", gx, gy, gz);
-    if ((long long)gx * gy * gz > (1ll << 31) / gamer::NCOMP - 1) return fail(GAMER_EINVAL, "too many groups for one launch");
+    if (gamer::ghost_fill_ctas(gx, gy, gz) > (1ll << 31) - 1) return fail(GAMER_EINVAL, "too many groups for one launch");
     if ((bc_x | bc_y | bc_z) & ~1) return fail(GAMER_EINVAL, "boundary flags must be 0 (periodic) or 1 (keep)");
     return GAMER_OK;
 }
@@ -229,9 +229,8 @@ int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int
     if (d_interior == nullptr || d_padded == nullptr) return fail(GAMER_EINVAL, "NULL pointer");
     if (!aligned16(d_interior) || !aligned16(d_padded)) return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
     g_err[0] = '\0';
-    const long long n = (long long)gx * gy * gz;
     gamer::BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
-    gamer::ghost_fill_kernel<<<(unsigned int)(n * gamer::NCOMP), gamer::GF_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
+    gamer::ghost_fill_kernel<<<(unsigned int)gamer::ghost_fill_ctas(gx, gy, gz), gamer::GF_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
         d_interior, d_padded, geo);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "ghost_fill launch: %s", cudaGetErrorString(e));
@@ -265,7 +264,7 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
         cfl_dt_kernel<<<1, 1, 0, stream>>>(d_work, cfl, dh, d_dt_log ? d_dt_log + s : nullptr);
         fn<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, make_const(0.f, dh, gamma), nullptr,
                                                         nullptr, d_work + 1);
-        ghost_fill_kernel<<<(unsigned int)(n * NCOMP), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
+        ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "run_uniform: %s", cudaGetErrorString(e));

@@ -21,44 +21,76 @@ struct BoxGeom {
 // neighbours; rows whose y or z lies beyond the box come from the y/z neighbours (periodic) or are re-read from the
 // padded array itself ("keep") — and then written out as one contiguous, 16-byte-aligned block with 128-bit stores.
 constexpr int GF_THREADS = 256;
+constexpr int GF_TILE = 4;
+// number of CTAs that ghost_fill_kernel needs for a box of gx x gy x gz groups
+inline long long ghost_fill_ctas(int gx, int gy, int gz) {
+    auto up = [](int a) { return (long long)((a + GF_TILE - 1) / GF_TILE); };
+    return up(gx) * up(gy) * up(gz) * GF_TILE * GF_TILE * GF_TILE * NCOMP;
+}
 __global__ void __launch_bounds__(GF_THREADS)
 ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded, BoxGeom geo) {
     __shared__ __align__(16) float tile[VAR_FLOATS];
-    const long long g = blockIdx.x / NCOMP;
+    // CTAs walk the box in 4 x 4 x 4 tiles of groups, so that the neighbours whose interiors a group reads are
+    // handled close in time and the reads hit L2 (in plain group order the z neighbours are gx*gy groups apart)
     const int v = blockIdx.x % NCOMP;
-    const int kx = (int)(g % geo.gx), ky = (int)((g / geo.gx) % geo.gy), kz = (int)(g / ((long long)geo.gx * geo.gy));
+    const long long q = blockIdx.x / NCOMP;
+    const int ntx = (geo.gx + GF_TILE - 1) / GF_TILE, nty = (geo.gy + GF_TILE - 1) / GF_TILE;
+    const long long tile_id = q / (GF_TILE * GF_TILE * GF_TILE);
+    const int w = (int)(q % (GF_TILE * GF_TILE * GF_TILE));
+    const int kx = (int)(tile_id % ntx) * GF_TILE + w % GF_TILE;
+    const int ky = (int)((tile_id / ntx) % nty) * GF_TILE + (w / GF_TILE) % GF_TILE;
+    const int kz = (int)(tile_id / ((long long)ntx * nty)) * GF_TILE + w / (GF_TILE * GF_TILE);
+    if (kx >= geo.gx || ky >= geo.gy || kz >= geo.gz) return;
+    const long long g = ((long long)kz * geo.gy + ky) * geo.gx + kx;
     float* dst = padded + (g * NCOMP + v) * (long long)VAR_FLOATS;
-    // x neighbours (group coordinate, or -1 = beyond a "keep" end)
+    // Per padded y and z: offset (in floats) of the source row inside `interior`, or -1 = beyond a "keep" end.  The
+    // index arithmetic is done once per CTA here, not once per cell (the first version was bound by it).
+    __shared__ long long off_y[NP], off_z[NP];
+    constexpr long long GS = (long long)NCOMP * PS * PS * PS;     // floats per group of `interior`
+    if (threadIdx.x < 2 * NP) {
+        const bool is_z = threadIdx.x >= NP;
+        const int p = threadIdx.x - (is_z ? NP : 0);
+        const int k = is_z ? kz : ky, nk = is_z ? geo.gz : geo.gy, keep_flag = is_z ? geo.bc[2] : geo.bc[1];
+        int c = p - NG, sk = k;
+        bool keep = false;
+        if (c < 0) { c += PS; sk = k > 0 ? k - 1 : nk - 1; keep = (k == 0 && keep_flag); }
+        else if (c >= PS) { c -= PS; sk = k < nk - 1 ? k + 1 : 0; keep = (k == nk - 1 && keep_flag); }
+        const long long off = is_z ? ((long long)sk * geo.gy * geo.gx) * GS + c * (PS * PS)
+                                   : ((long long)sk * geo.gx) * GS + c * PS;
+        (is_z ? off_z : off_y)[p] = keep ? -1 : off;
+    }
+    __syncthreads();
+    // x: own group, left and right neighbour (or -1 = beyond a "keep" end)
     const int kxl = kx > 0 ? kx - 1 : (geo.bc[0] ? -1 : geo.gx - 1);
     const int kxr = kx < geo.gx - 1 ? kx + 1 : (geo.bc[0] ? -1 : 0);
-    for (int t = threadIdx.x; t < NP * NP * 8; t += GF_THREADS) {
-        const int row = t >> 3, part = t & 7;          // parts 0..3: interior quarter; 4: left ghosts; 5: right ghosts
-        if (part > 5) continue;
-        const int y = row % NP, z = row / NP;
-        // source group and interior index along y and z
-        int ys = y - NG, zs = z - NG, sky = ky, skz = kz;
-        bool keep = false;
-        if (ys < 0) { ys += PS; sky = ky > 0 ? ky - 1 : geo.gy - 1; keep |= (ky == 0 && geo.bc[1]); }
-        else if (ys >= PS) { ys -= PS; sky = ky < geo.gy - 1 ? ky + 1 : 0; keep |= (ky == geo.gy - 1 && geo.bc[1]); }
-        if (zs < 0) { zs += PS; skz = kz > 0 ? kz - 1 : geo.gz - 1; keep |= (kz == 0 && geo.bc[2]); }
-        else if (zs >= PS) { zs -= PS; skz = kz < geo.gz - 1 ? kz + 1 : 0; keep |= (kz == geo.gz - 1 && geo.bc[2]); }
-        float* trow = tile + row * NP;
-        const int skx = part < 4 ? kx : (part == 4 ? kxl : kxr);
-        const int x0 = part < 4 ? NG + 4 * part : (part == 4 ? 0 : NG + PS);          // first padded x of this part
-        const int n = part < 4 ? 4 : NG;
-        if (keep || skx < 0) {
-            for (int i = 0; i < n; ++i) trow[x0 + i] = dst[row * NP + x0 + i];
+    const float* const src_c = interior + kx * GS + v * (PS * PS * PS);
+    const float* const src_l = kxl < 0 ? nullptr : interior + kxl * GS + v * (PS * PS * PS) + (PS - NG);
+    const float* const src_r = kxr < 0 ? nullptr : interior + kxr * GS + v * (PS * PS * PS) - (PS + NG);
+    // (1) the 16 cells x = 3..18 of every row: four 128-bit loads per row
+#pragma unroll 4
+    for (int t = threadIdx.x; t < NP * NP * 4; t += GF_THREADS) {
+        const int row = t >> 2, part = t & 3;
+        const int z = row / NP, y = row - z * NP;
+        const long long oy = off_y[y], oz = off_z[z];
+        float* trow = tile + row * NP + NG + 4 * part;
+        float4 q;
+        if (oy >= 0 && oz >= 0) {
+            q = *reinterpret_cast<const float4*>(src_c + oz + oy + 4 * part);
         } else {
-            const float* src = interior + ((((long long)skz * geo.gy + sky) * geo.gx + skx) * NCOMP + v) * (long long)(PS * PS * PS) +
-                               (zs * PS + ys) * PS;
-            if (part < 4) {
-                const float4 q = *reinterpret_cast<const float4*>(src + 4 * part);
-                trow[x0] = q.x; trow[x0 + 1] = q.y; trow[x0 + 2] = q.z; trow[x0 + 3] = q.w;
-            } else {
-                const int xs = part == 4 ? PS - NG : 0;
-                for (int i = 0; i < NG; ++i) trow[x0 + i] = src[xs + i];
-            }
+            const float* d = dst + row * NP + NG + 4 * part;
+            q = make_float4(d[0], d[1], d[2], d[3]);
         }
+        trow[0] = q.x; trow[1] = q.y; trow[2] = q.z; trow[3] = q.w;
+    }
+    // (2) the ghost cells x = 0..2 (left neighbour's cells 13..15) and x = 19..21 (right neighbour's cells 0..2)
+#pragma unroll 2
+    for (int t = threadIdx.x; t < NP * NP * 2 * NG; t += GF_THREADS) {
+        const int row = t / (2 * NG), j = t - row * (2 * NG);
+        const int z = row / NP, y = row - z * NP;
+        const long long oy = off_y[y], oz = off_z[z];
+        const int x = j < NG ? j : PS + j;                        // padded x: 0..2 or 19..21
+        const float* sx = j < NG ? src_l : src_r;                 // sx[x] is the source cell of padded x
+        tile[row * NP + x] = (oy >= 0 && oz >= 0 && sx != nullptr) ? sx[oz + oy + x] : dst[row * NP + x];
     }
     __syncthreads();
     for (int i = threadIdx.x; i < VAR_FLOATS / 4; i += GF_THREADS)
