@@ -317,6 +317,7 @@ def run_ours(args):
                        steps=e2e_steps, ms_per_step=1e3 * wall / e2e_steps, groups_per_chunk=chunk, n_streams=ns,
                        h2d_gbs=h_in.numel() * 4 * e2e_steps / wall / 1e9, api="gamer_hydro_pipeline_run (pinned host)")
             del h_in, h_out
+            hydro.gamer_hydro_pipeline_release()
         except Exception as ex:      # e.g. not enough pinnable host memory
             e2e = dict(value=None, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0, error=str(ex)[:200])
 

@@ -84,12 +84,18 @@ GAMER_API size_t gamer_hydro_face_flux_floats(long long n_groups);
  * into chunks of groups_per_chunk (the paper's N_g) that travel round-robin through n_streams (N_s) CUDA streams,
  * each doing one host->device copy, one kernel, one device->host copy, so that copies overlap kernels of other
  * chunks.  h_in / h_out: host pointers, same layouts as d_in / d_out; page-locked (pinned) memory is needed for the
- * copies to overlap — pageable memory works but serialises.  The call allocates and frees its own device staging
- * buffers (n_streams * groups_per_chunk groups), runs on the current device and is SYNCHRONOUS: on return h_out is
- * complete.  1 <= n_streams <= 16, groups_per_chunk >= 1, else GAMER_EINVAL. */
+ * copies to overlap — pageable memory works but serialises.  The call owns its device staging buffers
+ * (n_streams * groups_per_chunk groups) and streams: it allocates them on first use, keeps them for the next call
+ * (grown if that call needs more) and gamer_hydro_pipeline_release() frees them.  It runs on the current device and is
+ * SYNCHRONOUS: on return h_out is complete.  Concurrent calls from several host threads are serialised.
+ * 1 <= n_streams <= 16, groups_per_chunk >= 1, else GAMER_EINVAL. */
 GAMER_API int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups, int ghost,
                              float dt, float dh, float gamma, int backward,
                              long long groups_per_chunk, int n_streams);
+
+/* Frees the streams and staging buffers that gamer_hydro_pipeline_run keeps on the current device (after waiting for
+ * them).  A no-op if there are none. */
+GAMER_API int gamer_hydro_pipeline_release(void);
 
 /* NEXT-3 — device-side preparation step for a SINGLE-LEVEL tiling ("ghost zones ... filled by directly
  * copying from the sibling patches"; :430-432, :647 name this CPU step the bottleneck of the code).  gx*gy*gz groups tile

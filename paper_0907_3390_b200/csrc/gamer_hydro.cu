@@ -52,6 +52,17 @@ struct DeviceInfo {
 std::mutex g_mu;
 DeviceInfo g_dev[64];
 
+// Streams and device staging buffers of gamer_hydro_pipeline_run, per device, kept between calls.
+struct Staging {
+    cudaStream_t stream[16] = {};
+    float* d_in[16] = {};
+    float* d_out[16] = {};
+    size_t in_bytes[16] = {};
+    size_t out_bytes[16] = {};
+};
+std::mutex g_pipe_mu;
+Staging g_staging[64];
+
 // SM count of the current device and the opt-in to 208 KB of dynamic shared memory, once per device and kernel.
 int prepare(const void* fn, int key, int smem_bytes, int* sm_count) {
     int dev = 0;
@@ -172,15 +183,33 @@ int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups
 
     const size_t in_bytes = (size_t)groups_per_chunk * gamer::GROUP_IN_FLOATS * sizeof(float);
     const size_t out_bytes = (size_t)groups_per_chunk * gamer::GROUP_OUT_FLOATS * sizeof(float);
-    std::vector<cudaStream_t> streams((size_t)n_streams, nullptr);
-    std::vector<float*> d_in((size_t)n_streams, nullptr), d_out((size_t)n_streams, nullptr);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= 64) return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    // The streams and staging buffers are kept between calls (allocating 3 x 150 MB costs ~10 % of a config-5 call)
+    // and grown when a call needs more; gamer_hydro_pipeline_release() frees them.  Calls are serialised per process.
+    std::lock_guard<std::mutex> lk(g_pipe_mu);
+    Staging& st = g_staging[dev];
     int status = GAMER_OK;
-    cudaError_t e = cudaSuccess;
     for (int s = 0; s < n_streams && status == GAMER_OK; ++s) {
-        e = cudaStreamCreateWithFlags(&streams[s], cudaStreamNonBlocking);
-        if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); break; }
-        e = cudaMalloc(&d_in[s], in_bytes);
-        if (e == cudaSuccess) e = cudaMalloc(&d_out[s], out_bytes);
+        if (st.stream[s] == nullptr) {
+            e = cudaStreamCreateWithFlags(&st.stream[s], cudaStreamNonBlocking);
+            if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); break; }
+        }
+        if (st.in_bytes[s] < in_bytes) {
+            if (st.d_in[s]) cudaFree(st.d_in[s]);
+            st.d_in[s] = nullptr;
+            st.in_bytes[s] = 0;
+            e = cudaMalloc(&st.d_in[s], in_bytes);
+            if (e == cudaSuccess) st.in_bytes[s] = in_bytes;
+        }
+        if (e == cudaSuccess && st.out_bytes[s] < out_bytes) {
+            if (st.d_out[s]) cudaFree(st.d_out[s]);
+            st.d_out[s] = nullptr;
+            st.out_bytes[s] = 0;
+            e = cudaMalloc(&st.d_out[s], out_bytes);
+            if (e == cudaSuccess) st.out_bytes[s] = out_bytes;
+        }
         if (e != cudaSuccess) {
             status = fail(e == cudaErrorMemoryAllocation ? GAMER_ENOMEM : GAMER_ECUDA, "cudaMalloc of staging buffers: %s",
                           cudaGetErrorString(e));
@@ -193,26 +222,40 @@ int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups
         const int s = (int)(c % n_streams);
         const long long g0 = c * groups_per_chunk;
         const long long ng = (n_groups - g0) < groups_per_chunk ? (n_groups - g0) : groups_per_chunk;
-        e = cudaMemcpyAsync(d_in[s], h_in + g0 * gamer::GROUP_IN_FLOATS, (size_t)ng * gamer::GROUP_IN_FLOATS * sizeof(float),
-                            cudaMemcpyHostToDevice, streams[s]);
+        e = cudaMemcpyAsync(st.d_in[s], h_in + g0 * gamer::GROUP_IN_FLOATS,
+                            (size_t)ng * gamer::GROUP_IN_FLOATS * sizeof(float), cudaMemcpyHostToDevice, st.stream[s]);
         if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaMemcpyAsync H2D: %s", cudaGetErrorString(e)); break; }
-        status = launch(d_in[s], d_out[s], ng, dt, dh, gamma, backward, nullptr, nullptr, streams[s]);
+        status = launch(st.d_in[s], st.d_out[s], ng, dt, dh, gamma, backward, nullptr, nullptr, st.stream[s]);
         if (status != GAMER_OK) break;
-        e = cudaMemcpyAsync(h_out + g0 * gamer::GROUP_OUT_FLOATS, d_out[s],
-                            (size_t)ng * gamer::GROUP_OUT_FLOATS * sizeof(float), cudaMemcpyDeviceToHost, streams[s]);
+        e = cudaMemcpyAsync(h_out + g0 * gamer::GROUP_OUT_FLOATS, st.d_out[s],
+                            (size_t)ng * gamer::GROUP_OUT_FLOATS * sizeof(float), cudaMemcpyDeviceToHost, st.stream[s]);
         if (e != cudaSuccess) { status = fail(GAMER_ECUDA, "cudaMemcpyAsync D2H: %s", cudaGetErrorString(e)); break; }
     }
     for (int s = 0; s < n_streams; ++s) {
-        if (streams[s]) {
-            e = cudaStreamSynchronize(streams[s]);
+        if (st.stream[s]) {
+            e = cudaStreamSynchronize(st.stream[s]);
             if (e != cudaSuccess && status == GAMER_OK)
                 status = fail(GAMER_ECUDA, "cudaStreamSynchronize: %s", cudaGetErrorString(e));
         }
-        if (d_in[s]) cudaFree(d_in[s]);
-        if (d_out[s]) cudaFree(d_out[s]);
-        if (streams[s]) cudaStreamDestroy(streams[s]);
     }
     return status;
+}
+
+int gamer_hydro_pipeline_release(void) {
+    int dev = 0;
+    const cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= 64) return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    std::lock_guard<std::mutex> lk(g_pipe_mu);
+    Staging& st = g_staging[dev];
+    for (int s = 0; s < 16; ++s) {
+        if (st.stream[s]) cudaStreamSynchronize(st.stream[s]);
+        if (st.d_in[s]) cudaFree(st.d_in[s]);
+        if (st.d_out[s]) cudaFree(st.d_out[s]);
+        if (st.stream[s]) cudaStreamDestroy(st.stream[s]);
+    }
+    st = Staging();
+    g_err[0] = '\0';
+    return GAMER_OK;
 }
 
 static int check_box(int gx, int gy, int gz, int bc_x, int bc_y, int bc_z) {

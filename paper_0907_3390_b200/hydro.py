@@ -45,6 +45,8 @@ def lib():
         L.gamer_hydro_face_flux_floats.argtypes = [ll]
         L.gamer_hydro_pipeline_run.restype = ci
         L.gamer_hydro_pipeline_run.argtypes = [vp, vp, ll, ci, cf, cf, cf, ci, ll, ci]
+        L.gamer_hydro_pipeline_release.restype = ci
+        L.gamer_hydro_pipeline_release.argtypes = []
         L.gamer_hydro_ghost_fill.restype = ci
         L.gamer_hydro_ghost_fill.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, vp]
         L.gamer_hydro_run_uniform.restype = ci
@@ -128,6 +130,14 @@ def gamer_hydro_pipeline_run(h_in, h_out, n_groups, ghost, dt, dh, gamma, backwa
     """Host buffers in, host buffers out (pinned for overlap), synchronous (Fig.5)."""
     rc = lib().gamer_hydro_pipeline_run(_ptr(h_in), _ptr(h_out), n_groups, ghost, dt, dh, gamma, int(backward),
                                         groups_per_chunk, n_streams)
+    if check:
+        _check(rc)
+    return rc
+
+
+def gamer_hydro_pipeline_release(check=True):
+    """Free the streams and staging buffers that gamer_hydro_pipeline_run keeps between calls."""
+    rc = lib().gamer_hydro_pipeline_release()
     if check:
         _check(rc)
     return rc

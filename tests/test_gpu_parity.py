@@ -210,6 +210,15 @@ def test_pipeline_matches_direct_call_with_ragged_chunks():
         h_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32).pin_memory()
         hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, c["dt"], c["dh"], c["gamma"], 0, chunk, ns)
         assert np.array_equal(h_out.numpy(), direct), (chunk, ns)
+    # the staging buffers are kept between calls (grown above from 7 to 300 groups); release and run again
+    before = torch.cuda.mem_get_info()[0]
+    hydro.gamer_hydro_pipeline_release()
+    assert torch.cuda.mem_get_info()[0] > before
+    hydro.gamer_hydro_pipeline_release()          # a no-op when nothing is held
+    h_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32).pin_memory()
+    hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, c["dt"], c["dh"], c["gamma"], 1, 50, 2)
+    assert np.array_equal(h_out.numpy(), gpu_advance(inp, c["dt"], c["dh"], c["gamma"], backward=1))
+    hydro.gamer_hydro_pipeline_release()
 
 
 def test_runs_on_a_side_stream():
