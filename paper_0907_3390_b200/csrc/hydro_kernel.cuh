@@ -285,6 +285,7 @@ __device__ __forceinline__ void named_bar_arrive(int id, int n_threads) {
 
 // Named barriers of the forward pass (0 is __syncthreads).  LOADER_WARP has no z rows and only 4 x rows.
 constexpr int LOADER_WARP = BLOCK_THREADS / 32 - 1;
+static_assert(BLOCK_THREADS == 512, "16 warps: 16 x tasks (the last one 4 rows wide), 11 y tasks, 8 z tasks");
 constexpr int BAR_ZFREE = 1;                      // + c: the 256 z threads arrive, the loader warp syncs
 constexpr int BAR_FULL = 1 + N_CHUNK;             // + c: the loader warp arrives, the x warps that need chunk c sync
 static_assert(BAR_FULL + N_CHUNK <= 16, "named barriers");

@@ -159,6 +159,26 @@ def test_face_flux_and_group_maxspeed():
             assert np.abs(face[:, :, :, v] - o_face[:, :, :, v]).max() <= 1e-5 * scale, (backward, v)
 
 
+@pytest.mark.parametrize("backward", [0, 1])
+def test_optional_outputs_over_several_groups_per_cta(backward):
+    """350 different groups: every persistent CTA takes two or three in a row, so the per-group CFL reduction (slots
+    that rotate with the iteration) and the face-flux addressing are exercised across group boundaries."""
+    rng = np.random.default_rng(42 + backward)
+    c = W.config3()
+    idx = rng.permutation(c["inp"].shape[0])[:350]
+    inp = np.ascontiguousarray(c["inp"][idx])
+    out, face, speed = gpu_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward, face=True, speed=True)
+    o_out, o_face, o_speed = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward,
+                                                  want_face_flux=True, want_maxspeed=True, n_threads=NT)
+    assert W.parity_error(out, o_out, c["gamma"])["max_rel"] <= TOL32
+    np.testing.assert_allclose(speed, o_speed, rtol=2e-6)
+    for v in range(5):
+        scale = np.abs(o_face[:, :, :, v]).max()
+        assert np.abs(face[:, :, :, v] - o_face[:, :, :, v]).max() <= 1e-5 * scale, v
+    # the optional outputs do not change the main one
+    assert np.array_equal(out, gpu_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward))
+
+
 @pytest.mark.parametrize("axis", [0, 1, 2])
 def test_config2_sod_teacher_forced_and_free_running(axis):
     """Config 2 (128 groups, 128x64x64, gamma=1.4, 100 steps at CFL 0.5, readings R12-R16).
