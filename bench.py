@@ -340,6 +340,28 @@ def run_ours(args):
             optional_outputs[name] = dict(ns_per_group=e0.elapsed_time(e1) / 5 * 1e6 / n)
         del d_face, d_speed
 
+    # NEXT-4 (reported separately): the forward pass in double precision on the first 8192 groups of the workload
+    f64 = None
+    if rank == 0 and not args.no_ghost_fill:
+        n64 = min(n, 8192)
+        d_in64 = d_in[:n64].double()
+        d_out64 = torch.empty((n64, 5, 16, 16, 16), dtype=torch.float64, device=device)
+        d_scr = torch.empty(hydro.gamer_hydro_f64_scratch_doubles(), dtype=torch.float64, device=device)
+        for _ in range(2):
+            hydro.gamer_hydro_advance_f64(d_in64, d_out64, n64, 3, dt, dh, gamma, d_scr, stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(5):
+            hydro.gamer_hydro_advance_f64(d_in64, d_out64, n64, 3, dt, dh, gamma, d_scr, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms64 = e0.elapsed_time(e1) / 5
+        gbs64 = n64 * 2 * BYTES_PER_GROUP / (ms64 * 1e-3) / 1e9
+        f64 = dict(api="gamer_hydro_advance_f64", n_groups=n64, ns_per_group=ms64 * 1e6 / n64,
+                   value=n64 * CELLS_PER_GROUP / (ms64 * 1e-3), unit=UNIT, dtype="f64",
+                   hbm_achieved_gbs=gbs64, hbm_frac=gbs64 / peaks["hbm_gbs"], algorithmic_bytes=n64 * 2 * BYTES_PER_GROUP)
+        del d_in64, d_out64, d_scr
+
     # NEXT-3 (reported separately, not part of the step): device-side ghost fill of the same batch seen as a periodic
     # box of groups — reads every interior once, writes every padded group once.  It overwrites d_in, so it runs last.
     ghost_fill = None
@@ -374,7 +396,7 @@ def run_ours(args):
                                 launch=info),
                     roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
                     cpu_baseline=cpu_baseline, e2e=e2e, gpu_launches=args.steps, clocks=clocks,
-                    next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs,
+                    next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs, next4_f64=f64,
                     parity_spot_check_max_rel=parity)
         print(json.dumps(line))
     if dist is not None:

@@ -30,16 +30,32 @@ constexpr int PS = 16;
 constexpr int NG = 3;
 constexpr int NP = PS + 2 * NG;   // 22
 
-struct GasConst {
-    float gm1;      // gamma - 1
-    float ggm1;     // gamma (gamma - 1)
-    float kq;       // (dt/dh) / 4
-    float kh;       // (dt/dh) / 2
-    float kq_gm1;   // kq (gamma - 1)
-    float kq_sg;    // kq sqrt(gamma (gamma - 1))
-    float dh;       // cell size            } only read when the time step comes from device memory
-    float sg;       // sqrt(gamma (gamma-1)) }
+// T = float is the paper's precision and the hot path; T = double is the variant the paper switches to
+// for its convergence tests (:452).  The arithmetic is written once, on the overloads below.
+template <class T>
+struct GasConstT {
+    T gm1;      // gamma - 1
+    T ggm1;     // gamma (gamma - 1)
+    T kq;       // (dt/dh) / 4
+    T kh;       // (dt/dh) / 2
+    T kq_gm1;   // kq (gamma - 1)
+    T kq_sg;    // kq sqrt(gamma (gamma - 1))
+    T dh;       // cell size            } only read when the time step comes from device memory
+    T sg;       // sqrt(gamma (gamma-1)) }
 };
+using GasConst = GasConstT<float>;
+
+// explicitly rounded (never contracted) operations and fused multiply-add, per precision
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float fma_rn(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float abs_of(float a) { return fabsf(a); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ double abs_of(double a) { return fabs(a); }
 
 __device__ __forceinline__ float rcp_fast(float x) {
 #ifdef GAMER_EXP_NOMUFU      // timing experiment only (results are garbage)
@@ -60,80 +76,101 @@ __device__ __forceinline__ float sqrt_fast(float x) {
 #endif
 }
 
+// Double precision: hardware seed (relative error 2^-20) and two Newton steps — about 1 ulp, a fifth of the
+// instructions of an IEEE division or square root.
+__device__ __forceinline__ double rcp_fast(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(r, fma(-x, r, 1.0), r);
+    r = fma(r, fma(-x, r, 1.0), r);
+    return r;
+}
+__device__ __forceinline__ double sqrt_fast(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = fma(y * fma(-x * y, y, 1.0), 0.5, y);          // y <- y + y (1 - x y^2) / 2
+    y = fma(y * fma(-x * y, y, 1.0), 0.5, y);
+    const double s = x * y;
+    return fma(fma(-s, s, x), 0.5 * y, s);             // s <- s + (x - s^2) y / 2   (x > 0: P > 0 is the caller's duty)
+}
+
 // What a cell at time t contributes to the half step of its neighbours and of itself (all times q = (dt/dh)/4).
-struct HalfCoef {
-    float cp;     // q (c + v)
-    float cm;     // q (c - v)
-    float sig;    // 1 - 2 q c
-    float P;      // q P
-    float Pv;     // q P v
+template <class T>
+struct HalfCoefT {
+    T cp;     // q (c + v)
+    T cm;     // q (c - v)
+    T sig;    // 1 - 2 q c
+    T P;      // q P
+    T Pv;     // q P v
 };
 
 // u = (rho, m_n, m_t1, m_t2, e), m_n normal to the sweep.  c = |v_n| + c_s (reading R1), P from all three
 // momenta (Eqs.4-5, reading R2).
-__device__ __forceinline__ HalfCoef half_coef(const float (&u)[NCOMP], const GasConst& gc) {
-    HalfCoef h;
-    const float rinv = rcp_fast(u[0]);
-    const float v = __fmul_rn(u[1], rinv);
-    float q = __fmul_rn(u[2], u[2]);
-    q = fmaf(u[3], u[3], q);
-    q = fmaf(u[1], u[1], q);
-    const float hk = __fmul_rn(0.5f, rinv);
-    const float eint = fmaf(-q, hk, u[4]);                          // e - rho v^2 / 2
-    h.P = __fmul_rn(gc.kq_gm1, eint);
-    const float s = sqrt_fast(__fmul_rn(eint, rinv));
-    const float vq = __fmul_rn(gc.kq, v);
-    const float c = __fadd_rn(fabsf(vq), __fmul_rn(gc.kq_sg, s));   // q (|v| + c_s)
-    h.cp = __fadd_rn(c, vq);
-    h.cm = __fsub_rn(c, vq);
-    h.sig = fmaf(-2.0f, c, 1.0f);
-    h.Pv = __fmul_rn(h.P, v);
+template <class T>
+__device__ __forceinline__ HalfCoefT<T> half_coef(const T (&u)[NCOMP], const GasConstT<T>& gc) {
+    HalfCoefT<T> h;
+    const T rinv = rcp_fast(u[0]);
+    const T v = mul_rn(u[1], rinv);
+    T q = mul_rn(u[2], u[2]);
+    q = fma_rn(u[3], u[3], q);
+    q = fma_rn(u[1], u[1], q);
+    const T hk = mul_rn(T(0.5), rinv);
+    const T eint = fma_rn(-q, hk, u[4]);                          // e - rho v^2 / 2
+    h.P = mul_rn(gc.kq_gm1, eint);
+    const T s = sqrt_fast(mul_rn(eint, rinv));
+    const T vq = mul_rn(gc.kq, v);
+    const T c = add_rn(abs_of(vq), mul_rn(gc.kq_sg, s));   // q (|v| + c_s)
+    h.cp = add_rn(c, vq);
+    h.cm = sub_rn(c, vq);
+    h.sig = fma_rn(T(-2), c, T(1));
+    h.Pv = mul_rn(h.P, v);
     return h;
 }
 
 // Cell-centred G^R = c u + F = u (c + v) + (0, P, 0, 0, P v) and G^L = c u - F = u (c - v) - (0, P, 0, 0, P v) of the
 // midpoint state (2 F^R and 2 F^L of Eq.8).  Explicit intrinsics: no FMA contraction across cells.
-__device__ __forceinline__ void cell_split_flux(const float (&u)[NCOMP], const GasConst& gc, float (&gr)[NCOMP],
-                                                float (&gl)[NCOMP]) {
-    const float rinv = rcp_fast(u[0]);
-    const float v = __fmul_rn(u[1], rinv);
-    float q = __fmul_rn(u[2], u[2]);
-    q = fmaf(u[3], u[3], q);
-    q = fmaf(u[1], u[1], q);
-    const float hk = __fmul_rn(0.5f, rinv);
-    const float eint = fmaf(-q, hk, u[4]);
-    const float P = __fmul_rn(gc.gm1, eint);
-    const float cs = sqrt_fast(__fmul_rn(__fmul_rn(gc.ggm1, eint), rinv));
-    const float c = __fadd_rn(fabsf(v), cs);
-    const float cp = __fadd_rn(c, v), cm = __fsub_rn(c, v);
-    const float Pv = __fmul_rn(P, v);
-    gr[0] = __fmul_rn(u[0], cp);
-    gr[1] = fmaf(u[1], cp, P);
-    gr[2] = __fmul_rn(u[2], cp);
-    gr[3] = __fmul_rn(u[3], cp);
-    gr[4] = fmaf(u[4], cp, Pv);
-    gl[0] = __fmul_rn(u[0], cm);
-    gl[1] = fmaf(u[1], cm, -P);
-    gl[2] = __fmul_rn(u[2], cm);
-    gl[3] = __fmul_rn(u[3], cm);
-    gl[4] = fmaf(u[4], cm, -Pv);
+template <class T>
+__device__ __forceinline__ void cell_split_flux(const T (&u)[NCOMP], const GasConstT<T>& gc, T (&gr)[NCOMP],
+                                                T (&gl)[NCOMP]) {
+    const T rinv = rcp_fast(u[0]);
+    const T v = mul_rn(u[1], rinv);
+    T q = mul_rn(u[2], u[2]);
+    q = fma_rn(u[3], u[3], q);
+    q = fma_rn(u[1], u[1], q);
+    const T hk = mul_rn(T(0.5), rinv);
+    const T eint = fma_rn(-q, hk, u[4]);
+    const T P = mul_rn(gc.gm1, eint);
+    const T cs = sqrt_fast(mul_rn(mul_rn(gc.ggm1, eint), rinv));
+    const T c = add_rn(abs_of(v), cs);
+    const T cp = add_rn(c, v), cm = sub_rn(c, v);
+    const T Pv = mul_rn(P, v);
+    gr[0] = mul_rn(u[0], cp);
+    gr[1] = fma_rn(u[1], cp, P);
+    gr[2] = mul_rn(u[2], cp);
+    gr[3] = mul_rn(u[3], cp);
+    gr[4] = fma_rn(u[4], cp, Pv);
+    gl[0] = mul_rn(u[0], cm);
+    gl[1] = fma_rn(u[1], cm, -P);
+    gl[2] = mul_rn(u[2], cm);
+    gl[3] = mul_rn(u[3], cm);
+    gl[4] = fma_rn(u[4], cm, -Pv);
 }
 
 // base + a b / (a + b) if a b > 0, else base     (sgn = +1)   |   base - a b / (a + b) ...   (sgn = -1)
 // A select on the sign of the product, never a mask (reading R6).
-template <int SGN>
-__device__ __forceinline__ float limited(float base, float a, float b) {
-    const float p = a * b;
-    const float r = rcp_fast(a + b);
-    const float x = fmaf(SGN > 0 ? p : -p, r, base);
-    return p > 0.f ? x : base;
+template <int SGN, class T>
+__device__ __forceinline__ T limited(T base, T a, T b) {
+    const T p = a * b;
+    const T r = rcp_fast(a + b);
+    const T x = fma_rn(SGN > 0 ? p : -p, r, base);
+    return p > T(0) ? x : base;
 }
 
 // Marches one row.  Src::load(n, ua, ub) fetches cells n (even) and n+1 of the row, row-local component order.
 // Sink must provide:
-//   template <int ODD> void cell(int j, const float (&u)[5])   updated cell j = 3..18 (ODD = j & 1, static),
+//   template <int ODD> void cell(int j, const T (&u)[5])   updated cell j = 3..18 (ODD = j & 1, static),
 //                                            row-local component order
-//   void face(int p, const float (&f)[5])   true flux F^{t+dt/2} through interface 2|3 (p=0), 10|11 (1), 18|19 (2);
+//   void face(int p, const T (&f)[5])   true flux F^{t+dt/2} through interface 2|3 (p=0), 10|11 (1), 18|19 (2);
 //                                            called only if WANT_FACE
 // A Sink may overwrite the row in place at index j (the march never reads cell j again).
 // Gate: gate.acquire(n) is called before cells n, n+1 are read and gate.release(n) once they are in registers.
@@ -148,55 +185,55 @@ __device__ __forceinline__ float limited(float base, float a, float b) {
 // cannot fill the issue slots: latching cost 5 registers and one drain step per row and gained 3.4 %.
 // Steps 0..7 fill the pipeline (PH = n, statically pruned); steps 8..21 are identical and run as a rolled loop
 // (PH = 7), so that the code stays resident in the instruction cache; a last half step drains cell 18.
-template <bool WANT_FACE, class Sink>
+template <bool WANT_FACE, class Sink, class T = float>
 struct RowMarch {
-    float u1[NCOMP], u2[NCOMP], u3[NCOMP], u4[NCOMP];   // u_{n-1} .. u_{n-4} (the originals, kept for Eqs.13-14)
-    float sig1, cp1, P1, Pv1;                  // 1 - 2 q c, q (c+v), q P, q P v of cell n-1
-    float cp2, P2, Pv2;                        // ... of cell n-2
-    float uhl[NCOMP];                          // midpoint state of cell m = n-2 (latched by the previous step)
-    float gr2_prev[NCOMP], gl2_prev[NCOMP];    // midpoint G^R, G^L of cell m-1
-    float ar1[NCOMP], al1[NCOMP];              // G^R_{m-1} - G^R_{m-2}, G^L_{m-1} - G^L_{m-2}
-    float xr_prev[NCOMP];                      // 2 F^R through (m-2|m-1), limited
-    float fh_prev[NCOMP];                      // 2 F^h through (m-3|m-2)
+    T u1[NCOMP], u2[NCOMP], u3[NCOMP], u4[NCOMP];   // u_{n-1} .. u_{n-4} (the originals, kept for Eqs.13-14)
+    T sig1, cp1, P1, Pv1;                  // 1 - 2 q c, q (c+v), q P, q P v of cell n-1
+    T cp2, P2, Pv2;                        // ... of cell n-2
+    T uhl[NCOMP];                          // midpoint state of cell m = n-2 (latched by the previous step)
+    T gr2_prev[NCOMP], gl2_prev[NCOMP];    // midpoint G^R, G^L of cell m-1
+    T ar1[NCOMP], al1[NCOMP];              // G^R_{m-1} - G^R_{m-2}, G^L_{m-1} - G^L_{m-2}
+    T xr_prev[NCOMP];                      // 2 F^R through (m-2|m-1), limited
+    T fh_prev[NCOMP];                      // 2 F^h through (m-3|m-2)
 
     // stage B of step n: everything that follows from the midpoint state of cell m = n-2; new value of cell j = n-4
     template <int PH, int ODD>
-    __device__ __forceinline__ void stage_b(int n, const GasConst& gc, Sink& sink) {
+    __device__ __forceinline__ void stage_b(int n, const GasConstT<T>& gc, Sink& sink) {
         if (PH >= 3) {
-            float gr2[NCOMP], gl2[NCOMP];
+            T gr2[NCOMP], gl2[NCOMP];
             cell_split_flux(uhl, gc, gr2, gl2);                             // (d), cell m
             if (PH >= 4) {                                                  // m >= 2
-                float ar0[NCOMP], al0[NCOMP];
+                T ar0[NCOMP], al0[NCOMP];
 #pragma unroll
                 for (int k = 0; k < NCOMP; ++k) {
                     ar0[k] = gr2[k] - gr2_prev[k];
                     al0[k] = gl2[k] - gl2_prev[k];
                 }
-                float xr[NCOMP];
+                T xr[NCOMP];
                 if (PH >= 5) {                                              // m >= 3: (e) right-moving, (m-1|m)
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) xr[k] = limited<+1>(gr2_prev[k], ar1[k], ar0[k]);
                 }
                 if (PH >= 6) {                                              // m >= 4: (e) left-moving, (m-2|m-1)
-                    float fh[NCOMP];
+                    T fh[NCOMP];
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) {
-                        const float xl = limited<-1>(gl2_prev[k], al0[k], al1[k]);
+                        const T xl = limited<-1>(gl2_prev[k], al0[k], al1[k]);
                         fh[k] = xr_prev[k] - xl;
                     }
                     if (WANT_FACE) {
                         const int i = n - 4;                                // interface (i | i+1), i = m-2
                         if (i == NG - 1 || i == NG + PS / 2 - 1 || i == NG + PS - 1) {
-                            float ff[NCOMP];
+                            T ff[NCOMP];
 #pragma unroll
-                            for (int k = 0; k < NCOMP; ++k) ff[k] = 0.5f * fh[k];
+                            for (int k = 0; k < NCOMP; ++k) ff[k] = T(0.5) * fh[k];
                             sink.face(i == NG - 1 ? 0 : (i == NG + PS - 1 ? 2 : 1), ff);
                         }
                     }
                     if (PH >= 7) {                                          // m >= 5: (f) cell j = m-2 = n-4
-                        float un[NCOMP];
+                        T un[NCOMP];
 #pragma unroll
-                        for (int k = 0; k < NCOMP; ++k) un[k] = fmaf(-gc.kh, fh[k] - fh_prev[k], u4[k]);
+                        for (int k = 0; k < NCOMP; ++k) un[k] = fma_rn(-gc.kh, fh[k] - fh_prev[k], u4[k]);
                         sink.template cell<ODD>(n - 4, un);
                     }
 #pragma unroll
@@ -219,15 +256,15 @@ struct RowMarch {
 
     // stage A of step n: coefficients of cell n (a), midpoint state of cell n-1 (b)+(c) into the latch; window shift
     template <int PH>
-    __device__ __forceinline__ void stage_a(const float (&u)[NCOMP], const GasConst& gc) {
-        const HalfCoef h = half_coef(u, gc);
+    __device__ __forceinline__ void stage_a(const T (&u)[NCOMP], const GasConstT<T>& gc) {
+        const HalfCoefT<T> h = half_coef(u, gc);
         if (PH >= 2) {
-            const float dP = __fsub_rn(P2, h.P), dPv = __fsub_rn(Pv2, h.Pv);
+            const T dP = sub_rn(P2, h.P), dPv = sub_rn(Pv2, h.Pv);
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) {
-                float b = (k == 1) ? fmaf(sig1, u1[k], dP) : ((k == 4) ? fmaf(sig1, u1[k], dPv) : __fmul_rn(sig1, u1[k]));
-                b = fmaf(cp2, u2[k], b);
-                uhl[k] = fmaf(h.cm, u[k], b);
+                T b = (k == 1) ? fma_rn(sig1, u1[k], dP) : ((k == 4) ? fma_rn(sig1, u1[k], dPv) : mul_rn(sig1, u1[k]));
+                b = fma_rn(cp2, u2[k], b);
+                uhl[k] = fma_rn(h.cm, u[k], b);
             }
         }
 #pragma unroll
@@ -242,8 +279,8 @@ struct RowMarch {
     }
 
     template <int PH0, int PH1, class Src, class Gate>
-    __device__ __forceinline__ void pair(Src& src, int n, const GasConst& gc, Sink& sink, Gate& gate) {
-        float ua[NCOMP], ub[NCOMP];
+    __device__ __forceinline__ void pair(Src& src, int n, const GasConstT<T>& gc, Sink& sink, Gate& gate) {
+        T ua[NCOMP], ub[NCOMP];
         gate.acquire(n);
         src.load(n, ua, ub);
         gate.release(n);
@@ -254,7 +291,7 @@ struct RowMarch {
     }
 
     template <class Src, class Gate>
-    __device__ __forceinline__ void run(Src& src, const GasConst& gc, Sink& sink, Gate& gate) {
+    __device__ __forceinline__ void run(Src& src, const GasConstT<T>& gc, Sink& sink, Gate& gate) {
         pair<0, 1>(src, 0, gc, sink, gate);
         pair<2, 3>(src, 2, gc, sink, gate);
         pair<4, 5>(src, 4, gc, sink, gate);

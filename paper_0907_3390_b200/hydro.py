@@ -51,6 +51,10 @@ def lib():
         L.gamer_hydro_ghost_fill.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, vp]
         L.gamer_hydro_run_uniform.restype = ci
         L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
+        L.gamer_hydro_advance_f64.restype = ci
+        L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, vp, vp]
+        L.gamer_hydro_f64_scratch_doubles.restype = ctypes.c_size_t
+        L.gamer_hydro_f64_scratch_doubles.argtypes = []
         L.gamer_hydro_launch_info.restype = ci
         L.gamer_hydro_launch_info.argtypes = [ll] + [ctypes.POINTER(ci)] * 4
         L.gamer_last_error.restype = ctypes.c_char_p
@@ -157,6 +161,19 @@ def gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, 
     """n_steps of {CFL dt on the device, forward pass, ghost fill} without leaving the device."""
     rc = lib().gamer_hydro_run_uniform(_ptr(d_padded), _ptr(d_interior), gx, gy, gz, bc_x, bc_y, bc_z, n_steps, cfl, dh,
                                        gamma, _ptr(d_work), _ptr(d_dt_log), _stream_ptr(stream))
+    if check:
+        _check(rc)
+    return rc
+
+
+def gamer_hydro_f64_scratch_doubles():
+    return int(lib().gamer_hydro_f64_scratch_doubles())
+
+
+def gamer_hydro_advance_f64(d_in, d_out, n_groups, ghost, dt, dh, gamma, d_scratch, stream=None, check=True):
+    """Forward pass in double precision; d_scratch: gamer_hydro_f64_scratch_doubles() doubles."""
+    rc = lib().gamer_hydro_advance_f64(_ptr(d_in), _ptr(d_out), n_groups, ghost, dt, dh, gamma, _ptr(d_scratch),
+                                       _stream_ptr(stream))
     if check:
         _check(rc)
     return rc

@@ -1,0 +1,92 @@
+"""NEXT-4: the forward pass in double precision, against the fp64 oracle.
+
+Tolerance: the kernel and the oracle order the same ~80 roundings per row update differently (FMA contraction,
+G = c u + F against w = F/c), so they differ by a few hundred eps64 of a cell's own scale; the ill-conditioned cells of
+config 5 (cold cells next to a hot spot) amplify that as they do in fp32 (146 eps32 there).  Bar: 1e-11
+with the metric of reading R11 — five orders of magnitude below the fp32 bar."""
+import ctypes
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_0907_3390_b200 import hydro
+from paper_0907_3390_b200 import workloads as W
+
+TOL = 1e-11
+
+
+def test_f64_argument_validation_needs_no_device():
+    L = hydro.lib()
+    buf = (ctypes.c_double * 64)()
+    a16 = (ctypes.addressof(buf) + 15) & ~15
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 2, 0.1, 1.0, 1.4, a16, None) == hydro.GAMER_EUNSUPPORTED
+    assert L.gamer_hydro_advance_f64(a16, a16, -1, 3, 0.1, 1.0, 1.4, a16, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.4, None, None) == hydro.GAMER_EINVAL      # scratch
+    assert L.gamer_hydro_advance_f64(a16, a16 + 8, 1, 3, 0.1, 1.0, 1.4, a16, None) == hydro.GAMER_EINVAL    # alignment
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 0.0, 1.4, a16, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.0, a16, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64(None, None, 0, 3, 0.1, 1.0, 1.4, None, None) == hydro.GAMER_OK
+
+
+def gpu_advance_f64(inp, dt, dh, gamma):
+    import torch
+    n = inp.shape[0]
+    d_in = torch.from_numpy(np.ascontiguousarray(inp, np.float64)).cuda()
+    d_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float64, device="cuda")
+    d_scr = torch.empty(hydro.gamer_hydro_f64_scratch_doubles(), dtype=torch.float64, device="cuda")
+    hydro.gamer_hydro_advance_f64(d_in, d_out, n, 3, dt, dh, gamma, d_scr)
+    torch.cuda.synchronize()
+    return d_out.cpu().numpy()
+
+
+@pytest.mark.gpu
+def test_f64_config1_and_its_fp32_neighbour():
+    c = W.config1()
+    inp = c["inp"].astype(np.float64)
+    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"])
+    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64)
+    e = W.parity_error(got, ref, c["gamma"])
+    assert e["max_rel"] <= TOL, e
+    assert e["max_rel"] > 0 or np.array_equal(got, ref)
+    # and the fp32 product stays within its own bar of this result
+    o32 = oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"])
+    assert W.parity_error(o32.astype(np.float64), got, c["gamma"])["max_rel"] <= 1e-4
+
+
+@pytest.mark.gpu
+def test_f64_uniform_state_bit_exact():
+    u = np.empty((2, 5, 22, 22, 22), np.float64)
+    for g, vals in enumerate(([1.3, 0.4, -0.2, 0.7, 2.9], [1000.0, 3e3, -2e3, 1e3, 1e5])):
+        for i in range(5):
+            u[g, i] = vals[i]
+    out = gpu_advance_f64(u, 0.002, 1 / 128, 5 / 3)
+    for g in range(2):
+        for i in range(5):
+            assert (out[g, i] == u[g, i, 0, 0, 0]).all()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [1, 149, 300])
+def test_f64_ragged_group_counts(n):
+    rng = np.random.default_rng(n)
+    c = W.config3()
+    inp = c["inp"][rng.integers(0, c["inp"].shape[0], n)].astype(np.float64)
+    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"])
+    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64, n_threads=8)
+    assert W.parity_error(got, ref, c["gamma"])["max_rel"] <= TOL
+
+
+@pytest.mark.gpu
+def test_f64_config4_and_config5_samples():
+    c = W.config4()
+    inp = c["inp"][::64].astype(np.float64)
+    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"])
+    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64, n_threads=8)
+    assert W.parity_error(got, ref, c["gamma"])["max_rel"] <= TOL
+    hot = W.config5_hot_groups()[:6]
+    c5 = W.config5(list(hot) + [0, 1])
+    inp = c5["inp"].astype(np.float64)
+    got = gpu_advance_f64(inp, c5["dt"], c5["dh"], c5["gamma"])
+    ref = oracle.hydro_advance(inp, c5["dt"], c5["dh"], c5["gamma"], dtype=np.float64, n_threads=8)
+    assert W.parity_error(got, ref, c5["gamma"])["max_rel"] <= TOL
