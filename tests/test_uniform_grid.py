@@ -141,3 +141,30 @@ def test_gpu_run_uniform_config2_sod(axis):
     x = (np.arange(128) + 0.5) * dh
     rho_e, _, _ = riemann_exact.sample((x - 0.5) / dts.sum(), 1, 0, 1, 0.125, 0, 0.1, gamma)
     assert np.mean(np.abs(rho - rho_e)) <= 1.0e-2
+
+
+@pytest.mark.gpu
+def test_gpu_run_uniform_one_step_equals_advance_plus_ghost_fill():
+    """The driver's kernel reads dt from device memory and forms the dt-dependent constants itself: with the dt it
+    logged, the plain entry points must give the same bits."""
+    import torch
+    c = W.config1()
+    grid = (2, 2, 2)
+    d_p = torch.from_numpy(c["inp"]).cuda()
+    d_i = torch.empty((8, 5, 16, 16, 16), dtype=torch.float32, device="cuda")
+    d_work = torch.zeros(4, dtype=torch.float32, device="cuda")
+    d_log = torch.zeros(1, dtype=torch.float32, device="cuda")
+    hydro.gamer_hydro_run_uniform(d_p, d_i, 2, 2, 2, 0, 0, 0, 1, 0.5, c["dh"], c["gamma"], d_work, d_log)
+    torch.cuda.synchronize()
+    dt = float(d_log.cpu().numpy()[0])
+    ref_speed = oracle.max_signal_speed(c["inp"], c["gamma"])
+    assert abs(dt - 0.5 * c["dh"] / ref_speed) <= 2e-6 * dt
+    d_in = torch.from_numpy(c["inp"]).cuda()
+    d_out = torch.empty_like(d_i)
+    hydro.gamer_hydro_advance(d_in, d_out, 8, 3, dt, c["dh"], c["gamma"])
+    d_p2 = torch.full_like(d_p, float("nan"))
+    hydro.gamer_hydro_ghost_fill(d_out, d_p2, 2, 2, 2)
+    torch.cuda.synchronize()
+    assert torch.equal(d_out.view(torch.int32), d_i.view(torch.int32))
+    assert torch.equal(d_p2.view(torch.int32), d_p.view(torch.int32))
+    assert np.array_equal(d_p.cpu().numpy(), oracle.ghost_fill(d_i.cpu().numpy(), grid))
