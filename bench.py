@@ -382,6 +382,25 @@ def run_ours(args):
                           peak=peaks["hbm_gbs"], unit="GB/s", frac=gf_gbs / peaks["hbm_gbs"],
                           algorithmic_bytes=n * BYTES_PER_GROUP)
 
+    # NEXT-3 driver: whole steps (dt, forward pass, ghost fill) without leaving the device; runs last, it evolves d_in
+    run_uniform = None
+    if ghost_fill is not None:
+        box = ghost_fill["box_groups"]
+        d_work = torch.zeros(4 + n, dtype=torch.float32, device=device)
+        d_log = torch.zeros(4, dtype=torch.float32, device=device)
+        hydro.gamer_hydro_run_uniform(d_in, d_out, box[0], box[1], box[2], 0, 0, 0, 1, 0.5, dh, gamma, d_work, d_log,
+                                      stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        hydro.gamer_hydro_run_uniform(d_in, d_out, box[0], box[1], box[2], 0, 0, 0, 4, 0.5, dh, gamma, d_work, d_log,
+                                      stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ru_ms = e0.elapsed_time(e1) / 4
+        run_uniform = dict(api="gamer_hydro_run_uniform", steps=4, ms_per_step=ru_ms,
+                           value=n * CELLS_PER_GROUP / (ru_ms * 1e-3), unit=UNIT,
+                           dt_finite=bool(torch.isfinite(d_log).all().item()))
+
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cores = os.cpu_count() or 1
@@ -396,7 +415,7 @@ def run_ours(args):
                                 launch=info),
                     roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
                     cpu_baseline=cpu_baseline, e2e=e2e, gpu_launches=args.steps, clocks=clocks,
-                    next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs, next4_f64=f64,
+                    next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs, next4_f64=f64, next3_run_uniform=run_uniform,
                     parity_spot_check_max_rel=parity)
         print(json.dumps(line))
     if dist is not None:

@@ -109,12 +109,15 @@ GAMER_API int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, i
                            int bc_x, int bc_y, int bc_z, void* stream);
 
 /* NEXT-3 — multi-step driver on such a box, entirely on the device (no host round trip between steps).  Each of the
- * n_steps steps does: dt = cfl * dh / max over ALL padded cells of (c_s + max_i |v_i|) (Eq.30, PAPER.md:418-426;
- * fp32, reading R10); one forward pass gamer_hydro_advance(d_padded -> d_interior) with that dt (read from
- * device memory, constants formed exactly as on the host); gamer_hydro_ghost_fill(d_interior -> d_padded).  On return
- * (asynchronous on `stream`) d_padded holds the ghost-filled state after n_steps and d_interior its interiors.
- * d_work: >= 4 floats of device scratch, 16-byte aligned.  d_dt_log: optional device array of n_steps floats that
- * receives the dt of every step (NULL = off). */
+ * n_steps steps does: dt = cfl * dh / max over ALL padded cells of (c_s + max_i |v_i|) (Eq.30; fp32,
+ * DESIGN.md reading R10); one forward pass d_padded -> d_interior with that dt (read from device memory, constants
+ * formed exactly as on the host); gamer_hydro_ghost_fill(d_interior -> d_padded).  The maximum is taken in one pass
+ * over the initial state; from then on it is the maximum of the per-group speeds of the updated interiors that the
+ * hydro kernel writes as a by-product (:426: "a single floating-point value per patch group") and of the ghost cells
+ * beyond "keep" ends, which never change — the same set of cells.  On return (asynchronous on `stream`) d_padded holds
+ * the ghost-filled state after n_steps and d_interior its interiors.
+ * d_work: 4 + gx*gy*gz floats of device scratch, 16-byte aligned.  d_dt_log: optional device array of n_steps floats
+ * that receives the dt of every step (NULL = off). */
 GAMER_API int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, int gz,
                             int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dh, float gamma,
                             float* d_work, float* d_dt_log, void* stream);

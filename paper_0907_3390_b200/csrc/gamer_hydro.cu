@@ -289,25 +289,33 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     const long long n = (long long)gx * gy * gz;
     rc = validate(d_padded, d_interior, n, gamer::NG, 0.f, dh, gamma, 0, d_work, d_dt_log);
     if (rc != GAMER_OK) return rc;
-    if (d_work == nullptr) return fail(GAMER_EINVAL, "d_work must point to at least 4 floats of device memory");
+    if (d_work == nullptr) return fail(GAMER_EINVAL, "d_work must point to 4 + n_groups floats of device memory");
     if (n_steps < 0 || !(cfl > 0.f)) return fail(GAMER_EINVAL, "n_steps must be >= 0 and cfl > 0");
     g_err[0] = '\0';
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     using namespace gamer;
-    KernelFn fn = hydro_advance_kernel<false, false, false, true>;
+    KernelFn fn = hydro_advance_kernel<false, false, true, true>;       // forward, fused CFL speed, dt from the device
     int sm_count = 0;
     rc = prepare(reinterpret_cast<const void*>(fn), 8, SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
     const int grid = (int)(n < (long long)sm_count ? n : (long long)sm_count);
     const int red_grid = (int)(n < 4ll * sm_count ? n : 4ll * sm_count);
     BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
+    unsigned int* acc = reinterpret_cast<unsigned int*>(d_work);
+    float* d_speed = d_work + 4;
+    // Eq.30 over ALL padded cells (reading R10) costs one pass over the initial state.  After that the padded state
+    // is: updated interiors (their speed comes out of the hydro kernel, fused, per group), periodic ghost cells
+    // (copies of interiors) and ghost cells beyond "keep" ends (never change: their maximum is taken once, work[2]).
     cudaError_t e = cudaMemsetAsync(d_work, 0, 4 * sizeof(float), stream);
+    if (n_steps > 0 && e == cudaSuccess) {
+        if (bc_x | bc_y | bc_z) max_speed_kernel<<<red_grid, 256, 0, stream>>>(d_padded, n, gamma, acc + 2, geo, 1);
+        max_speed_kernel<<<red_grid, 256, 0, stream>>>(d_padded, n, gamma, acc, geo, 0);
+    }
     for (int s = 0; s < n_steps && e == cudaSuccess; ++s) {
-        // Eq.30 on the current padded state -> dt in d_work[1]; one forward pass with that dt; ghost refill
-        max_speed_kernel<<<red_grid, 256, 0, stream>>>(d_padded, n, gamma, reinterpret_cast<unsigned int*>(d_work));
         cfl_dt_kernel<<<1, 1, 0, stream>>>(d_work, cfl, dh, d_dt_log ? d_dt_log + s : nullptr);
         fn<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, make_const(0.f, dh, gamma), nullptr,
-                                                        nullptr, d_work + 1);
+                                                        d_speed, d_work + 1);
+        group_speed_max_kernel<<<(unsigned int)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, stream>>>(d_speed, n, acc);
         ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
         e = cudaGetLastError();
     }

@@ -97,15 +97,28 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
         reinterpret_cast<float4*>(dst)[i] = reinterpret_cast<const float4*>(tile)[i];
 }
 
-// max over ALL padded cells of all groups of c_s + max(|v_x|,|v_y|,|v_z|) (reading R10), as the bit pattern
-// of a non-negative float in *acc (atomicMax on unsigned: positive floats order like their bit patterns).
+// max of c_s + max(|v_x|,|v_y|,|v_z|) (Eq.30) as the bit pattern of a non-negative float in *acc (atomicMax on
+// unsigned: positive floats order like their bit patterns).  keep_only = 0: over ALL padded cells of all groups
+// (reading R10); keep_only = 1: only over the ghost cells beyond a "keep" end of the box, which no ghost
+// fill ever changes.
 __global__ void __launch_bounds__(256)
-max_speed_kernel(const float* __restrict__ padded, long long n_groups, float gamma, unsigned int* __restrict__ acc) {
+max_speed_kernel(const float* __restrict__ padded, long long n_groups, float gamma, unsigned int* __restrict__ acc,
+                 BoxGeom geo, int keep_only) {
     float best = 0.f;
     const float ggm1 = gamma * (gamma - 1.0f);
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
         const float* u = padded + g * (long long)GROUP_IN_FLOATS;
+        const int kx = (int)(g % geo.gx), ky = (int)((g / geo.gx) % geo.gy), kz = (int)(g / ((long long)geo.gx * geo.gy));
+        // per axis: padded indices below lo or from hi on lie beyond a "keep" end (lo = 0, hi = NP: none)
+        const int lox = geo.bc[0] && kx == 0 ? NG : 0, hix = geo.bc[0] && kx == geo.gx - 1 ? NG + PS : NP;
+        const int loy = geo.bc[1] && ky == 0 ? NG : 0, hiy = geo.bc[1] && ky == geo.gy - 1 ? NG + PS : NP;
+        const int loz = geo.bc[2] && kz == 0 ? NG : 0, hiz = geo.bc[2] && kz == geo.gz - 1 ? NG + PS : NP;
+        if (keep_only && lox == 0 && hix == NP && loy == 0 && hiy == NP && loz == 0 && hiz == NP) continue;
         for (int i = threadIdx.x; i < VAR_FLOATS; i += blockDim.x) {
+            if (keep_only) {
+                const int x = i % NP, y = (i / NP) % NP, z = i / (NP * NP);
+                if (x >= lox && x < hix && y >= loy && y < hiy && z >= loz && z < hiz) continue;
+            }
             const float rho = u[i], mx = u[VAR_FLOATS + i], my = u[2 * VAR_FLOATS + i], mz = u[3 * VAR_FLOATS + i],
                         e = u[4 * VAR_FLOATS + i];
             const float rinv = 1.0f / rho;
@@ -120,13 +133,25 @@ max_speed_kernel(const float* __restrict__ padded, long long n_groups, float gam
     if ((threadIdx.x & 31) == 0) atomicMax(acc, __float_as_uint(best));
 }
 
-// dt = cfl dh / speed; resets the accumulator for the next step.  work[0]: accumulator, work[1]: dt.
+// max over the per-group CFL speeds that the hydro kernel wrote (its fused NEXT-1 output) into *acc.
+__global__ void __launch_bounds__(256)
+group_speed_max_kernel(const float* __restrict__ group_speed, long long n_groups, unsigned int* __restrict__ acc) {
+    float best = 0.f;
+    for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups; g += (long long)gridDim.x * blockDim.x)
+        best = fmaxf(best, group_speed[g]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) best = fmaxf(best, __shfl_xor_sync(0xffffffffu, best, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(acc, __float_as_uint(best));
+}
+
+// dt = cfl dh / speed.  work[0]: speed accumulator (bits), work[1]: dt, work[2]: speed of the kept ghost cells (bits),
+// with which the accumulator starts the next step.
 __global__ void cfl_dt_kernel(float* __restrict__ work, float cfl, float dh, float* __restrict__ dt_log) {
-    const float speed = __uint_as_float(reinterpret_cast<unsigned int*>(work)[0]);
-    const float dt = cfl * dh / speed;
+    unsigned int* w = reinterpret_cast<unsigned int*>(work);
+    const float dt = cfl * dh / __uint_as_float(w[0]);
     work[1] = dt;
     if (dt_log) *dt_log = dt;
-    reinterpret_cast<unsigned int*>(work)[0] = 0u;
+    w[0] = w[2];
 }
 
 }  // namespace gamer

@@ -123,7 +123,7 @@ def test_gpu_run_uniform_config2_sod(axis):
     bc[axis] = 1
     d_p = torch.from_numpy(inp).cuda()
     d_i = torch.empty((inp.shape[0], 5, 16, 16, 16), dtype=torch.float32, device="cuda")
-    d_work = torch.zeros(4, dtype=torch.float32, device="cuda")
+    d_work = torch.zeros(4 + d_i.shape[0], dtype=torch.float32, device="cuda")
     d_log = torch.zeros(nsteps, dtype=torch.float32, device="cuda")
     hydro.gamer_hydro_run_uniform(d_p, d_i, gx, gy, gz, bc[0], bc[1], bc[2], nsteps, 0.5, dh, gamma, d_work, d_log)
     torch.cuda.synchronize()
@@ -152,7 +152,7 @@ def test_gpu_run_uniform_one_step_equals_advance_plus_ghost_fill():
     grid = (2, 2, 2)
     d_p = torch.from_numpy(c["inp"]).cuda()
     d_i = torch.empty((8, 5, 16, 16, 16), dtype=torch.float32, device="cuda")
-    d_work = torch.zeros(4, dtype=torch.float32, device="cuda")
+    d_work = torch.zeros(4 + d_i.shape[0], dtype=torch.float32, device="cuda")
     d_log = torch.zeros(1, dtype=torch.float32, device="cuda")
     hydro.gamer_hydro_run_uniform(d_p, d_i, 2, 2, 2, 0, 0, 0, 1, 0.5, c["dh"], c["gamma"], d_work, d_log)
     torch.cuda.synchronize()
