@@ -122,14 +122,15 @@ GAMER_API int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx
                             int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dh, float gamma,
                             float* d_work, float* d_dt_log, void* stream);
 
-/* NEXT-4 — the forward pass in DOUBLE precision (the paper switches to double for its convergence
- * tests).  Same operation, layouts and error conventions as gamer_hydro_advance with double arrays: d_in
- * [g][v][22][22][22] (425 920 B per group), d_out [g][v][16][16][16].  Reciprocals and square roots are IEEE.
- * d_scratch: device scratch of gamer_hydro_f64_scratch_doubles() doubles, 16-byte aligned, owned by the caller, not
- * shared between concurrent calls (one 5 x 22 x 16 x 16 block per SM: the group does not fit in shared memory and the
- * x,y-swept columns pass through it).  Forward order only; no optional outputs. */
+/* NEXT-4 — one pass in DOUBLE precision (the paper switches to double for its convergence tests).
+ * Same operation, layouts and error conventions as gamer_hydro_advance_ex with double arrays: d_in
+ * [g][v][22][22][22] (425 920 B per group), d_out [g][v][16][16][16]; backward = 0 sweeps x,y,z, 1 sweeps z,y,x.
+ * Reciprocals and square roots are accurate to about 1 ulp.  d_scratch: device scratch of
+ * gamer_hydro_f64_scratch_doubles() doubles, 16-byte aligned, owned by the caller, not shared between concurrent calls
+ * (one block per SM: the group does not fit in shared memory and the pass goes through it between sweeps).  No
+ * optional outputs. */
 GAMER_API int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost,
-                            double dt, double dh, double gamma, double* d_scratch, void* stream);
+                            double dt, double dh, double gamma, int backward, double* d_scratch, void* stream);
 /* Doubles of scratch gamer_hydro_advance_f64 needs on the current device; 0 (and an error message) without a device. */
 GAMER_API size_t gamer_hydro_f64_scratch_doubles(void);
 

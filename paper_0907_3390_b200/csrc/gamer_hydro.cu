@@ -335,11 +335,12 @@ size_t gamer_hydro_f64_scratch_doubles(void) {
 }
 
 int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost, double dt, double dh,
-                            double gamma, double* d_scratch, void* stream) {
+                            double gamma, int backward, double* d_scratch, void* stream) {
     if (ghost != gamer::NG)
         return fail(GAMER_EUNSUPPORTED, "ghost = %d: the 7-point stencil of the scheme fixes ghost = 3", ghost);
     if (n_groups < 0) return fail(GAMER_EINVAL, "n_groups = %lld < 0", n_groups);
     if (!(dh > 0.0) || !(dt >= 0.0) || !(gamma > 1.0)) return fail(GAMER_EINVAL, "need dh > 0, dt >= 0, gamma > 1");
+    if (backward != 0 && backward != 1) return fail(GAMER_EINVAL, "backward must be 0 or 1");
     if (n_groups > 0 && (d_in == nullptr || d_out == nullptr || d_scratch == nullptr))
         return fail(GAMER_EINVAL, "NULL input, output or scratch pointer");
     if (!aligned16(d_in) || !aligned16(d_out) || !aligned16(d_scratch))
@@ -347,8 +348,9 @@ int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_group
     g_err[0] = '\0';
     if (n_groups == 0) return GAMER_OK;
     int sm_count = 0;
-    const int rc = prepare(reinterpret_cast<const void*>(gamer::hydro_advance_f64_kernel), 9, gamer::F64_SMEM_BYTES,
-                           &sm_count);
+    using F64Fn = void (*)(const double*, double*, long long, gamer::GasConstT<double>, double*);
+    F64Fn fn = backward ? gamer::hydro_advance_f64_backward_kernel : gamer::hydro_advance_f64_kernel;
+    const int rc = prepare(reinterpret_cast<const void*>(fn), backward ? 10 : 9, gamer::F64_SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
     gamer::GasConstT<double> gc;
     const double k = dt / dh;
@@ -361,8 +363,8 @@ int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_group
     gc.kq_gm1 = gc.kq * gc.gm1;
     gc.kq_sg = gc.kq * gc.sg;
     const int grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
-    gamer::hydro_advance_f64_kernel<<<grid, gamer::F64_THREADS, gamer::F64_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(
-        d_in, d_out, n_groups, gc, d_scratch);
+    fn<<<grid, gamer::F64_THREADS, gamer::F64_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(d_in, d_out, n_groups, gc,
+                                                                                            d_scratch);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
     return GAMER_OK;

@@ -52,7 +52,7 @@ def lib():
         L.gamer_hydro_run_uniform.restype = ci
         L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
         L.gamer_hydro_advance_f64.restype = ci
-        L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, vp, vp]
+        L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp]
         L.gamer_hydro_f64_scratch_doubles.restype = ctypes.c_size_t
         L.gamer_hydro_f64_scratch_doubles.argtypes = []
         L.gamer_hydro_launch_info.restype = ci
@@ -170,10 +170,11 @@ def gamer_hydro_f64_scratch_doubles():
     return int(lib().gamer_hydro_f64_scratch_doubles())
 
 
-def gamer_hydro_advance_f64(d_in, d_out, n_groups, ghost, dt, dh, gamma, d_scratch, stream=None, check=True):
-    """Forward pass in double precision; d_scratch: gamer_hydro_f64_scratch_doubles() doubles."""
-    rc = lib().gamer_hydro_advance_f64(_ptr(d_in), _ptr(d_out), n_groups, ghost, dt, dh, gamma, _ptr(d_scratch),
-                                       _stream_ptr(stream))
+def gamer_hydro_advance_f64(d_in, d_out, n_groups, ghost, dt, dh, gamma, d_scratch, backward=0, stream=None,
+                            check=True):
+    """One pass in double precision; d_scratch: gamer_hydro_f64_scratch_doubles() doubles."""
+    rc = lib().gamer_hydro_advance_f64(_ptr(d_in), _ptr(d_out), n_groups, ghost, dt, dh, gamma, int(backward),
+                                       _ptr(d_scratch), _stream_ptr(stream))
     if check:
         _check(rc)
     return rc

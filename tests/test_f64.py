@@ -1,4 +1,4 @@
-"""NEXT-4: the forward pass in double precision, against the fp64 oracle.
+"""NEXT-4: the pass (both sweep orders) in double precision, against the fp64 oracle.
 
 Tolerance: the kernel and the oracle order the same ~80 roundings per row update differently (FMA contraction,
 G = c u + F against w = F/c), so they differ by a few hundred eps64 of a cell's own scale; the ill-conditioned cells of
@@ -20,60 +20,63 @@ def test_f64_argument_validation_needs_no_device():
     L = hydro.lib()
     buf = (ctypes.c_double * 64)()
     a16 = (ctypes.addressof(buf) + 15) & ~15
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 2, 0.1, 1.0, 1.4, a16, None) == hydro.GAMER_EUNSUPPORTED
-    assert L.gamer_hydro_advance_f64(a16, a16, -1, 3, 0.1, 1.0, 1.4, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.4, None, None) == hydro.GAMER_EINVAL      # scratch
-    assert L.gamer_hydro_advance_f64(a16, a16 + 8, 1, 3, 0.1, 1.0, 1.4, a16, None) == hydro.GAMER_EINVAL    # alignment
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 0.0, 1.4, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.0, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(None, None, 0, 3, 0.1, 1.0, 1.4, None, None) == hydro.GAMER_OK
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 2, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EUNSUPPORTED
+    assert L.gamer_hydro_advance_f64(a16, a16, -1, 3, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.4, 0, None, None) == hydro.GAMER_EINVAL      # scratch
+    assert L.gamer_hydro_advance_f64(a16, a16 + 8, 1, 3, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL    # alignment
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 0.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.0, 0, a16, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.4, 2, a16, None) == hydro.GAMER_EINVAL        # backward
+    assert L.gamer_hydro_advance_f64(None, None, 0, 3, 0.1, 1.0, 1.4, 1, None, None) == hydro.GAMER_OK
 
 
-def gpu_advance_f64(inp, dt, dh, gamma):
+def gpu_advance_f64(inp, dt, dh, gamma, backward=0):
     import torch
     n = inp.shape[0]
     d_in = torch.from_numpy(np.ascontiguousarray(inp, np.float64)).cuda()
     d_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float64, device="cuda")
     d_scr = torch.empty(hydro.gamer_hydro_f64_scratch_doubles(), dtype=torch.float64, device="cuda")
-    hydro.gamer_hydro_advance_f64(d_in, d_out, n, 3, dt, dh, gamma, d_scr)
+    hydro.gamer_hydro_advance_f64(d_in, d_out, n, 3, dt, dh, gamma, d_scr, backward=backward)
     torch.cuda.synchronize()
     return d_out.cpu().numpy()
 
 
 @pytest.mark.gpu
-def test_f64_config1_and_its_fp32_neighbour():
+@pytest.mark.parametrize("backward", [0, 1])
+def test_f64_config1_and_its_fp32_neighbour(backward):
     c = W.config1()
     inp = c["inp"].astype(np.float64)
-    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"])
-    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64)
+    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"], backward)
+    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64, backward=backward)
     e = W.parity_error(got, ref, c["gamma"])
     assert e["max_rel"] <= TOL, e
     assert e["max_rel"] > 0 or np.array_equal(got, ref)
     # and the fp32 product stays within its own bar of this result
-    o32 = oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"])
+    o32 = oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"], backward=backward)
     assert W.parity_error(o32.astype(np.float64), got, c["gamma"])["max_rel"] <= 1e-4
 
 
 @pytest.mark.gpu
-def test_f64_uniform_state_bit_exact():
+@pytest.mark.parametrize("backward", [0, 1])
+def test_f64_uniform_state_bit_exact(backward):
     u = np.empty((2, 5, 22, 22, 22), np.float64)
     for g, vals in enumerate(([1.3, 0.4, -0.2, 0.7, 2.9], [1000.0, 3e3, -2e3, 1e3, 1e5])):
         for i in range(5):
             u[g, i] = vals[i]
-    out = gpu_advance_f64(u, 0.002, 1 / 128, 5 / 3)
+    out = gpu_advance_f64(u, 0.002, 1 / 128, 5 / 3, backward)
     for g in range(2):
         for i in range(5):
             assert (out[g, i] == u[g, i, 0, 0, 0]).all()
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("n", [1, 149, 300])
-def test_f64_ragged_group_counts(n):
+@pytest.mark.parametrize("n,backward", [(1, 0), (149, 1), (300, 0), (300, 1)])
+def test_f64_ragged_group_counts(n, backward):
     rng = np.random.default_rng(n)
     c = W.config3()
     inp = c["inp"][rng.integers(0, c["inp"].shape[0], n)].astype(np.float64)
-    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"])
-    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64, n_threads=8)
+    got = gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"], backward)
+    ref = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], dtype=np.float64, n_threads=8, backward=backward)
     assert W.parity_error(got, ref, c["gamma"])["max_rel"] <= TOL
 
 
