@@ -93,3 +93,40 @@ def test_f64_config4_and_config5_samples():
     got = gpu_advance_f64(inp, c5["dt"], c5["dh"], c5["gamma"])
     ref = oracle.hydro_advance(inp, c5["dt"], c5["dh"], c5["gamma"], dtype=np.float64, n_threads=8)
     assert W.parity_error(got, ref, c5["gamma"])["max_rel"] <= TOL
+
+
+@pytest.mark.gpu
+def test_f64_acoustic_wave_converges_at_second_order_on_the_gpu():
+    """The paper's own accuracy test (double precision): a small-amplitude sound wave along the box
+    diagonal, K = (1,1,1)/sqrt 3, advanced by forward + backward pairs for one period on periodic boxes of 16^3, 32^3
+    and 64^3 cells; the paper reports L1 ~ N^-1.9.  Here the CUDA path is measured against the analytic solution (no
+    oracle involved): uniform background flow as in the oracle's pin (reading R20), ghost zones refilled
+    on the host."""
+    gamma, amp = 5.0 / 3.0, 1e-6
+    rho0, P0, cs, vb = 1.0, 3.0 / 5.0, 1.0, 0.3
+    speed = cs + np.sqrt(3.0) * vb
+
+    def run(n):
+        dh = 1.0 / n
+        c = (np.arange(n) + 0.5) * dh
+        Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+
+        def state(shift):
+            d = amp * np.sin(2 * np.pi * (X + Y + Z - shift))
+            vc = vb + cs * d / np.sqrt(3.0)
+            return W.conserved(rho0 * (1 + d), vc, vc, vc, P0 * (1 + gamma * d), gamma)
+
+        U = state(0.0)
+        grid = (n // 16,) * 3
+        t_end = 1.0 / (np.sqrt(3.0) * speed)
+        nsteps = int(np.ceil(t_end / (0.4 * dh / (cs + vb))))
+        nsteps += nsteps % 2
+        dt = t_end / nsteps
+        for s in range(nsteps):
+            U = W.groups_to_box(gpu_advance_f64(W.box_to_groups(U), dt, dh, gamma, backward=s % 2), grid)
+        return np.mean(np.abs(U[0] - state(np.sqrt(3.0) * speed * t_end)[0])) / amp
+
+    e = [run(n) for n in (16, 32, 64)]
+    slopes = [np.log2(e[i + 1] / e[i]) for i in range(2)]
+    assert all(-2.6 <= s <= -1.5 for s in slopes), (e, slopes)
+    assert e[2] < 0.02, e
