@@ -58,22 +58,14 @@ __device__ __forceinline__ double fma_rn(double a, double b, double c) { return 
 __device__ __forceinline__ double abs_of(double a) { return fabs(a); }
 
 __device__ __forceinline__ float rcp_fast(float x) {
-#ifdef GAMER_EXP_NOMUFU      // timing experiment only (results are garbage)
-    return __fmul_rn(x, 1.0001f);
-#else
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
-#endif
 }
 __device__ __forceinline__ float sqrt_fast(float x) {
-#ifdef GAMER_EXP_NOMUFU
-    return __fmul_rn(x, 0.9999f);
-#else
     float r;
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
-#endif
 }
 
 // Double precision: hardware seed (relative error 2^-20) and two Newton steps — about 1 ulp, a fifth of the
