@@ -22,6 +22,10 @@
 #define GAMER_MARCH_UNROLL 3     /* pairs of cells per loop body (measured: 1: 113.5, 2: 105.4, 3: 104.5, 4: 108.4 ns/group) */
 #endif
 
+#ifndef GAMER_MARCH_UNROLL_F64
+#define GAMER_MARCH_UNROLL_F64 1
+#endif
+
 namespace gamer {
 
 constexpr int MARCH_UNROLL = GAMER_MARCH_UNROLL;
@@ -288,7 +292,9 @@ struct RowMarch {
         pair<2, 3>(src, 2, gc, sink, gate);
         pair<4, 5>(src, 4, gc, sink, gate);
         pair<6, 7>(src, 6, gc, sink, gate);
-#pragma unroll MARCH_UNROLL
+        // pairs of cells per loop body: the fp64 step is 2.5 x as long, so its body is kept shorter
+        constexpr int UNROLL = sizeof(T) == 8 ? GAMER_MARCH_UNROLL_F64 : MARCH_UNROLL;
+#pragma unroll UNROLL
         for (int n = 8; n < NP; n += 2) pair<7, 7>(src, n, gc, sink, gate);
         stage_b<7, 0>(NP, gc, sink);            // drain: cell j = 18
     }
