@@ -24,7 +24,11 @@ def declared_symbols():
 def test_header_declares_the_survey_entry_points():
     syms = declared_symbols()
     for s in ("gamer_hydro_advance", "gamer_hydro_advance_ex", "gamer_hydro_in_floats", "gamer_hydro_out_floats",
-              "gamer_hydro_pipeline_run", "gamer_last_error", "gamer_version"):
+              "gamer_hydro_pipeline_run", "gamer_last_error", "gamer_version",
+              # beyond the survey's list: NEXT-2 size helper, NEXT-3, NEXT-4, pipeline housekeeping, reporting
+              "gamer_hydro_face_flux_floats", "gamer_hydro_ghost_fill", "gamer_hydro_run_uniform",
+              "gamer_hydro_advance_f64", "gamer_hydro_f64_scratch_doubles", "gamer_hydro_pipeline_release",
+              "gamer_hydro_launch_info"):
         assert s in syms
 
 
