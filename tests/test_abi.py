@@ -38,6 +38,11 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(L, s), s
 
 
+def test_python_binding_has_the_same_names():
+    for s in declared_symbols():
+        assert callable(getattr(hydro, s, None)), s
+
+
 def test_size_helpers():
     assert hydro.gamer_hydro_in_floats(1, 3) == 5 * 22 ** 3 == 53240
     assert hydro.gamer_hydro_in_floats(32768, 3) * 4 == 32768 * 212960
