@@ -137,14 +137,29 @@ def test_limited_flux_brackets_upwind_and_downwind_values():
 
 
 def test_linear_flux_profile_gives_central_flux():
-    """P-linear: where the cell-centred F^R (and F^L) vary linearly, phi(d,d)=d and Eqs.10-12 give the arithmetic mean
-    of the two neighbours.  Built on the density component with u = const velocity, const P: F^R_rho = rho (c+v)/2 is
-    linear in n when rho is linear and c is constant; c is constant only if c_s is, so use the limiter's defining
-    property on a row where rho, P scale together (c_s const) and v = 0 at the midpoint is not guaranteed —
-    instead check the scale-free statement directly through van_leer."""
-    for d in (0.3, -2.0, 1e-3):
-        a = 1.7
-        assert a + oracle.van_leer(d / 2, d / 2) == pytest.approx(0.5 * (a + (a + d)), rel=1e-15)
+    """P-linear at row level (Eqs.9-12, :145-162): where the cell-centred F^R and F^L vary linearly along the row,
+    phi(d, d) = d and the limited interface value is the arithmetic mean of the two neighbours.
+    Construction: gas at rest (v = 0), uniform pressure P, sqrt(rho) linear in n, and dt = 0 (the midpoint state is
+    the state itself).  Then c = c_s = sqrt(gamma P / rho) and, by Eq.8, the density components are
+    F^R_rho = F^L_rho = c rho / 2 = sqrt(gamma P rho) / 2 = alpha + beta n: linear.  Central values on both sides give
+    a time-centred mass flux F^R_{n+1/2} - F^L_{n+1/2} = 0 — the physical mass flux of a gas at rest — while the
+    first-order (phi = 0) flux is F^R_n - F^L_{n+1} = -beta.  The normal-momentum components are F^R = P/2,
+    F^L = -P/2 (uniform), so that flux is P with or without the limiter.
+    Catches a limiter that picks a wrong neighbour or drops the factor 2 of Eq.11 (the mean is then not central)."""
+    N, gamma, P = 22, G53, 0.6
+    alpha, beta = 0.5, 0.02
+    n = np.arange(N, dtype=np.float64)
+    rho = 4.0 * (alpha + beta * n) ** 2 / (gamma * P)                  # sqrt(gamma P rho)/2 = alpha + beta n
+    z = np.zeros(N)
+    u = W.conserved(rho, z, z, z, np.full(N, P), gamma)
+    _, fh = oracle.row_update(u, 0.0, gamma, want_flux=True)
+    _, fh1 = oracle.row_update(u, 0.0, gamma, limiter_on=0, want_flux=True)
+    sl = slice(2, N - 3)                                                # interfaces n + 1/2, n = 2..N-4
+    np.testing.assert_allclose(fh[0, sl], 0.0, atol=1e-15)             # second order: the exact mass flux, 0
+    np.testing.assert_allclose(fh1[0, sl], -beta, rtol=1e-12)          # first order: -beta (diffusion)
+    np.testing.assert_allclose(fh[1, sl], P, rtol=1e-14)
+    np.testing.assert_allclose(fh1[1, sl], P, rtol=1e-14)
+    assert (fh[2:4, sl] == 0).all()                                     # no transverse momentum, no flux of it
 
 
 # ------------------------------------------------------------------------------------------------ :178
@@ -273,8 +288,8 @@ def test_conservation_on_a_periodic_box(dtype, tol, backward):
 
 def test_face_fluxes_account_for_the_interior_change():
     """:340, :344-346 — the fluxes through the group's outer faces, as output, explain the change of the interior
-    totals: sum(out - in) = -k sum_d sum_faces (F_hi - F_lo).  The mid-plane flux explains each 8-cell patch layer of
-    the last sweep.  Catches a wrong plane index, a wrong variable mapping or transverse index order."""
+    totals: sum(out - in) = -k sum_d sum_faces (F_hi - F_lo).  Catches a wrong outer plane or variable mapping (sums over the face hide the transverse index
+    order: that is pinned by the two tests below)."""
     c = W.config1()
     inp = c["inp"].astype(np.float64)
     k = c["dt"] / c["dh"]
@@ -282,16 +297,6 @@ def test_face_fluxes_account_for_the_interior_change():
     change = (out - inp[:, :, 3:19, 3:19, 3:19]).sum(axis=(2, 3, 4))             # [G][5]
     net = (face[:, :, 2] - face[:, :, 0]).sum(axis=(1, 3, 4))                     # [G][5]
     np.testing.assert_allclose(change, -k * net, rtol=1e-9, atol=1e-10)
-    # last sweep (z, forward): lower patch layer k=0..7 changes by -k (F_mid - F_lo) relative to the state before the
-    # z sweep; check through the transverse index order instead: face z is indexed [j][i] like out[v][k][j][i]
-    out_b, face_b = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], backward=1, want_face_flux=True)
-    # backward pass: x is the last sweep; rebuild the pre-x-sweep interior column sums from the x faces [k][j]
-    dx_lo = -(k) * (face_b[:, 0, 1] - face_b[:, 0, 0])                            # [G][5][k][j] change of sum_{i<8}
-    dx_hi = -(k) * (face_b[:, 0, 2] - face_b[:, 0, 1])
-    tot = out_b.sum(axis=4)                                                       # [G][5][k][j]
-    lo, hi = out_b[..., :8].sum(axis=4), out_b[..., 8:].sum(axis=4)
-    # total over i before the x sweep = tot - (dx_lo + dx_hi); it must be the same whether rebuilt from halves
-    np.testing.assert_allclose((lo - dx_lo) + (hi - dx_hi), tot - (dx_lo + dx_hi), rtol=1e-12, atol=1e-12)
     # forward z-sweep layer statement against an independent route: advance with x,y only is not exposed, so use
     # mirror: reflecting z swaps the roles of planes 0 and 2 and negates the mass flux through them
     um = np.flip(inp, axis=2).copy()
@@ -299,6 +304,89 @@ def test_face_fluxes_account_for_the_interior_change():
     _, face_m = oracle.hydro_advance(um, c["dt"], c["dh"], c["gamma"], want_face_flux=True)
     np.testing.assert_allclose(face_m[:, 2, 0, 0], -face[:, 2, 2, 0], rtol=1e-10, atol=1e-12)
     np.testing.assert_allclose(face_m[:, 2, 1, 0], -face[:, 2, 1, 0], rtol=1e-10, atol=1e-12)
+
+
+def _two_axis_group(d, t, gamma, seed):
+    """One padded group whose state varies along the sweep axis d and along ONE transverse axis t only (axes
+    0:x, 1:y, 2:z), with a non-symmetric, non-periodic profile along both; all three velocity components non-zero."""
+    rng = np.random.default_rng(seed)
+    shape = [1, 1, 1]                                   # numpy order (z, y, x)
+    shape[2 - d] = 22
+    fd = lambda: rng.uniform(-1, 1, 22).reshape(shape)  # noqa: E731  profile along d
+    shape_t = [1, 1, 1]
+    shape_t[2 - t] = 22
+    ft = lambda: rng.uniform(-1, 1, 22).reshape(shape_t)  # noqa: E731  profile along t
+    full = np.ones((22, 22, 22))
+    rho = (1.0 + 0.2 * fd() + 0.2 * ft()) * full
+    vel = [(0.3 * fd() + 0.2 * ft() + 0.1) * full for _ in range(3)]
+    P = (1.0 + 0.2 * fd() + 0.2 * ft()) * full
+    return W.conserved(rho, vel[0], vel[1], vel[2], P, gamma)
+
+
+# (sweep axis d, transverse axis t that varies, backward flag).  The flag is chosen so that every sweep BEFORE d runs
+# along the third axis t', along which the state is uniform: such a sweep returns the state bit-exactly (P-uniform per
+# row), so the rows of the d sweep are rows of the input.  Forward order is x,y,z, backward z,y,x (:174-176).
+_FACE_CASES = [(0, 1, 0), (0, 2, 0), (1, 2, 0), (1, 0, 1), (2, 0, 1), (2, 1, 1)]
+
+
+@pytest.mark.parametrize("d,t,backward", _FACE_CASES)
+def test_face_flux_transverse_index_order(d, t, backward):
+    """:340, :344-346 and the header of the C ABI: face[d][p][v][b][a], (b, a) = the two transverse interior indices,
+    the one of the HIGHER axis number first (d=x: [k][j], d=y: [k][i], d=z: [j][i]); p = 0, 1, 2 are the interfaces
+    2|3, 10|11, 18|19 along d.  Pinned against oracle.row_update on the explicitly extracted row: the state varies
+    along d and along one transverse axis t only, so the flux through a face must vary with the index of t and with
+    nothing else.  A swapped (b, a) fails (the flux then varies along the wrong index)."""
+    gamma, dt, dh = G53, 1.0e-3, 1.0 / 64
+    k = dt / dh
+    u = _two_axis_group(d, t, gamma, 100 + 10 * d + t)
+    out, face = oracle.hydro_advance(u[None], dt, dh, gamma, backward=backward, want_face_flux=True)
+    face = face[0]
+    t1, t2 = (d + 1) % 3, (d + 2) % 3
+    comp = [0, 1 + d, 1 + t1, 1 + t2, 4]                 # row-local (rho, m_n, m_t1, m_t2, e) -> variable
+    planes = (2, 10, 18)
+    tp = 3 - d - t                                       # the uniform transverse axis
+    hi_is_t = t > tp                                     # is t the slower index b?
+    seen = []
+    for it in range(16):
+        idx = [0, 0, 0]                                  # (x, y, z) padded position of the row
+        idx[t] = it + 3
+        idx[tp] = 7 + 3                                  # any: the state does not depend on it
+        sel = [idx[2], idx[1], idx[0]]
+        sel[2 - d] = slice(None)
+        row = np.stack([u[(v,) + tuple(sel)] for v in comp])           # [5][22] row-local order
+        _, fh = oracle.row_update(row, k, gamma, want_flux=True)
+        for p in range(3):
+            for q in range(5):
+                want = fh[q, planes[p]]
+                got = face[d, p, comp[q], it, :] if hi_is_t else face[d, p, comp[q], :, it]
+                np.testing.assert_allclose(got, want, rtol=1e-13, atol=1e-14, err_msg=str((d, t, p, q, it)))
+        seen.append(fh[0, planes[1]])
+    assert np.ptp(seen) > 1e-3 * np.abs(seen).max()      # the flux does vary along t: the test can see a swap
+
+
+@pytest.mark.parametrize("backward", [0, 1])
+def test_face_flux_of_a_perturbed_column_sits_where_the_header_says(backward):
+    """Second, independent pin of the (b, a) order, all three axes and both sweep orders at once: perturb one
+    interior cell at (i0, j0, k0) with three different indices.  The domain of dependence of one pass is +-3 cells per
+    sweep, so the face-flux entries that change lie within 3 of (k0, j0) on x faces, (k0, i0) on y faces and (j0, i0)
+    on z faces — and, because the indices differ by more than 6, NOT around the transposed positions."""
+    c = W.config1()
+    inp = c["inp"][:1].astype(np.float64)
+    i0, j0, k0 = 2, 13, 8                                # interior indices (x, y, z), pairwise |difference| >= 5
+    pert = inp.copy()
+    pert[0, 0, k0 + 3, j0 + 3, i0 + 3] *= 1.05
+    pert[0, 4, k0 + 3, j0 + 3, i0 + 3] *= 1.05
+    _, f0 = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward, want_face_flux=True)
+    _, f1 = oracle.hydro_advance(pert, c["dt"], c["dh"], c["gamma"], backward=backward, want_face_flux=True)
+    changed = (f0[0] != f1[0]).any(axis=(1, 2))          # [d][b][a]
+    centre = {0: (k0, j0), 1: (k0, i0), 2: (j0, i0)}
+    for d in range(3):
+        bb, aa = np.nonzero(changed[d])
+        assert bb.size > 0, d
+        b0, a0 = centre[d]
+        # each sweep widens the set by 3 cells along its own axis: at most 3 along a transverse axis per earlier sweep
+        assert np.abs(bb - b0).max() <= 3 and np.abs(aa - a0).max() <= 3, (d, bb, aa)
+        assert changed[d][b0, a0]
 
 
 def test_group_max_speed_is_eq30_on_the_updated_interior():
