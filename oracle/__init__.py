@@ -181,9 +181,16 @@ def max_signal_speed(padded, gamma):
     return (np.sqrt(t(gamma) * p / rho) + v.max(axis=1)).max()
 
 
-def run_uniform(padded, grid, bc, n_steps, cfl, dh, gamma, n_threads=1):
-    """n_steps of {dt from Eq.30 over all padded cells; one forward pass; ghost refill} (DESIGN.md NEXT-3).
-    Returns (padded state, list of dt)."""
+def run_uniform(padded, grid, bc, n_steps, cfl, dh, gamma, n_threads=1, order=0):
+    """Multi-step loop on a single-level tiling (DESIGN.md NEXT-3).  Returns (padded state, list of dt).
+
+    order = 0: each step is {dt from Eq.30 over all padded cells (PAPER.md:418-426); one forward pass (x,y,z);
+               ghost refill}.
+    order = 1: the paper's full step: "a forward sweep in the order xyz, and follows a backward
+               sweep in the order zyx.  The same time step must be employed by these two sweeps": each step is {dt
+               from Eq.30; forward pass; ghost refill; backward pass (z,y,x) with the SAME dt; ghost refill} and
+               advances the state by 2 dt.  The next dt is evaluated after the backward sweep (:424)."""
+    assert order in (0, 1)
     u = np.array(padded, copy=True)
     t = u.dtype.type
     dts = []
@@ -191,5 +198,8 @@ def run_uniform(padded, grid, bc, n_steps, cfl, dh, gamma, n_threads=1):
         dt = t(cfl) * t(dh) / max_signal_speed(u, gamma)
         out = hydro_advance(u, dt, dh, gamma, n_threads=n_threads)
         u = ghost_fill(out, grid, bc, padded=u)
+        if order == 1:
+            out = hydro_advance(u, dt, dh, gamma, backward=1, n_threads=n_threads)
+            u = ghost_fill(out, grid, bc, padded=u)
         dts.append(float(dt))
     return u, dts
