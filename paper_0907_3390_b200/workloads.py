@@ -167,15 +167,11 @@ def config3(grid=(8, 8, 8)):
     return dict(name="config3", inp=inp, dt=cfl_dt(inp, dh, gamma), dh=dh, gamma=gamma, grid=grid)
 
 
-def config4(grid=(16, 16, 16)):
-    """4096 groups: ln rho Gaussian, sigma=2, shell-integrated spectrum E(k) = 4 pi k^2 P(k) ~ k^-3 (3-D power
-    P(k) ~ k^-5; DESIGN.md reading R17: with 3-D power ~ k^-3 adjacent cells differ by a factor e^1.2 rms, up to
-    e^6.6, and the floor-free scheme leaves the physical domain in both fp32 and fp64); P=rho^gamma;
-    v = 0.5(sqrt(1-a^2) g + a grad ln rho / rms), g ~ N(0,1) iid, a = 0.5."""
+def _clumpy_gas(grid, slope, name):
     gamma, dh, alpha = 5.0 / 3.0, 1.0 / 256.0, 0.5
     rng = rng_for(4)
     shp = (grid[0] * PS, grid[1] * PS, grid[2] * PS)
-    lnrho = 2.0 * gaussian_field(shp, -5.0, rng)
+    lnrho = 2.0 * gaussian_field(shp, slope, rng)
     lnrho -= lnrho.mean()
     rho = np.exp(lnrho)
     vel = []
@@ -186,7 +182,24 @@ def config4(grid=(16, 16, 16)):
         vel.append(0.5 * (np.sqrt(1.0 - alpha * alpha) * g + alpha * grad))
     U = conserved(rho, vel[0], vel[1], vel[2], rho ** gamma, gamma)
     inp = box_to_groups(U).astype(np.float32)
-    return dict(name="config4", inp=inp, dt=cfl_dt(inp, dh, gamma), dh=dh, gamma=gamma, grid=grid)
+    return dict(name=name, inp=inp, dt=cfl_dt(inp, dh, gamma), dh=dh, gamma=gamma, grid=grid)
+
+
+def config4(grid=(16, 16, 16)):
+    """4096 groups: ln rho Gaussian, sigma=2, shell-integrated spectrum E(k) = 4 pi k^2 P(k) ~ k^-3 (3-D power
+    P(k) ~ k^-5; DESIGN.md reading R17: with 3-D power ~ k^-3 adjacent cells differ by a factor e^1.2 rms, up to
+    e^6.6, and the floor-free scheme leaves the physical domain in both fp32 and fp64); P=rho^gamma;
+    v = 0.5(sqrt(1-a^2) g + a grad ln rho / rms), g ~ N(0,1) iid, a = 0.5.  Every group stays physical: this is the
+    config-4 input of the all-groups parity test and of the timing."""
+    return _clumpy_gas(grid, -5.0, "config4")
+
+
+def config4_literal(grid=(16, 16, 16)):
+    """Config 4 exactly as BASELINE.json / SURVEY.md 8(c)#17 word it: the same recipe with the 3-D power spectrum of
+    ln rho ~ |k|^-3.  The scheme has no floor (R7) and on this field part of the groups leave the physical
+    domain (rho <= 0 or P <= 0 somewhere along the pass) on the CPU oracle in fp32 and in fp64 alike; the tests
+    compare the CUDA path with the oracle on the groups that stay physical on both and state how many those are."""
+    return _clumpy_gas(grid, -3.0, "config4_literal")
 
 
 CONFIG5 = dict(n_groups=32768, grid=(32, 32, 32), gamma=5.0 / 3.0, dh=1.0 / 512.0, p_bg=1e-5, p_hot=1e3, frac=0.01)

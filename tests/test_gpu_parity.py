@@ -55,6 +55,31 @@ def check_parity(gpu, inp, dt, dh, gamma, backward=0):
     return e32, e64
 
 
+def face_flux_local_scale(inp, gamma):
+    """Per-element scale of the face fluxes [G][3][3][5][16][16]: c * s_v on the two cells next to the interface,
+    c = |v| + c_s, s_v = the R11 scale of variable v (rho, rho (|v| + c_s), e) — the size of |F^R| + |F^L| = c u there
+    (Eq.8), taken from the padded input (interfaces 2|3, 10|11, 18|19 along d)."""
+    u = np.asarray(inp, np.float64)
+    rho, mx, my, mz, e = (u[:, i] for i in range(5))
+    P = (gamma - 1.0) * (e - 0.5 * (mx * mx + my * my + mz * mz) / rho)
+    c = np.sqrt(mx * mx + my * my + mz * mz) / rho + np.sqrt(gamma * P / rho)
+    cell = np.stack([c * rho, c * c * rho, c * c * rho, c * c * rho, c * np.abs(e)], axis=1)      # [G][5][22][22][22]
+    G = u.shape[0]
+    scale = np.empty((G, 3, 3, 5, 16, 16))
+    for d in range(3):
+        ax = 4 - d                                            # numpy axis of x, y, z in [G][5][z][y][x]
+        for p, n in enumerate((2, 10, 18)):
+            pair = np.maximum(np.take(cell, n, axis=ax), np.take(cell, n + 1, axis=ax))        # [G][5][.][.] padded
+            scale[:, d, p] = pair[:, :, 3:19, 3:19]
+    return scale
+
+
+def assert_face_flux_parity(face, o_face, inp, gamma, tol=1e-5):
+    err = np.abs(face.astype(np.float64) - o_face) / face_flux_local_scale(inp, gamma)
+    assert np.isfinite(face).all()
+    assert err.max() <= tol, (err.max(), np.unravel_index(int(np.argmax(err)), err.shape))
+
+
 def test_library_is_the_cuda_one():
     info = hydro.gamer_hydro_launch_info(1000)
     assert info["block"] == 512 and info["smem_bytes"] >= 212960 and info["grid"] >= 100
@@ -153,10 +178,7 @@ def test_face_flux_and_group_maxspeed():
                                                       want_face_flux=True, want_maxspeed=True)
         assert W.parity_error(out, o_out, c["gamma"])["max_rel"] <= TOL32
         np.testing.assert_allclose(speed, o_speed, rtol=2e-6)
-        # flux of variable v scales like (|v|+c_s) * u_v: compare against the per-variable flux magnitude
-        for v in range(5):
-            scale = np.abs(o_face[:, :, :, v]).max()
-            assert np.abs(face[:, :, :, v] - o_face[:, :, :, v]).max() <= 1e-5 * scale, (backward, v)
+        assert_face_flux_parity(face, o_face, c["inp"], c["gamma"])       # per element, at the cell's own scale
 
 
 @pytest.mark.parametrize("backward", [0, 1])
@@ -172,9 +194,7 @@ def test_optional_outputs_over_several_groups_per_cta(backward):
                                                   want_face_flux=True, want_maxspeed=True, n_threads=NT)
     assert W.parity_error(out, o_out, c["gamma"])["max_rel"] <= TOL32
     np.testing.assert_allclose(speed, o_speed, rtol=2e-6)
-    for v in range(5):
-        scale = np.abs(o_face[:, :, :, v]).max()
-        assert np.abs(face[:, :, :, v] - o_face[:, :, :, v]).max() <= 1e-5 * scale, v
+    assert_face_flux_parity(face, o_face, inp, c["gamma"])
     # the optional outputs do not change the main one
     assert np.array_equal(out, gpu_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward))
 
