@@ -395,11 +395,11 @@ def run_ours(args):
         box = ghost_fill["box_groups"]
         d_work = torch.zeros(4 + n, dtype=torch.float32, device=device)
         d_log = torch.zeros(4, dtype=torch.float32, device=device)
-        hydro.gamer_hydro_run_uniform(d_in, d_out, box[0], box[1], box[2], 0, 0, 0, 1, 0.5, dh, gamma, d_work, d_log,
+        hydro.gamer_hydro_run_uniform(d_in, d_out, box[0], box[1], box[2], 0, 0, 0, 1, 0, 0.5, dh, gamma, d_work, d_log,
                                       stream=stream)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        hydro.gamer_hydro_run_uniform(d_in, d_out, box[0], box[1], box[2], 0, 0, 0, 4, 0.5, dh, gamma, d_work, d_log,
+        hydro.gamer_hydro_run_uniform(d_in, d_out, box[0], box[1], box[2], 0, 0, 0, 4, 0, 0.5, dh, gamma, d_work, d_log,
                                       stream=stream)
         e1.record(stream)
         torch.cuda.synchronize()

@@ -28,14 +28,16 @@
  *
  * OWNERSHIP: the caller owns every buffer.  `d_*` are DEVICE pointers (cudaMalloc or equivalent) valid on the
  * device of `stream`; `h_*` are HOST pointers.  Nothing is allocated, freed or synchronised by gamer_hydro_advance*:
- * they only enqueue work on `stream` (NULL = the legacy default stream).  `d_in` is never written.  Input and output
- * must not overlap.
+ * they only enqueue work on `stream` (NULL = the legacy default stream).  `d_in` is never written.  Input, outputs
+ * and scratch must not overlap (checked on the address ranges: results of finished groups are streamed out while later
+ * groups are still being read).
  *
  * ERRORS: every function returns GAMER_OK (0) or a negative gamer_status; nothing aborts or throws.  After a
  * failure gamer_last_error() returns a thread-local, statically stored, human-readable message.
  *   ghost != 3                                                        -> GAMER_EUNSUPPORTED  (stencil, :178)
  *   n_groups < 0; a required pointer NULL while n_groups > 0; a pointer not 16-byte aligned;
- *   !(dh > 0); !(dt >= 0); !(gamma > 1); backward not 0/1              -> GAMER_EINVAL
+ *   !(dh > 0); !(dt >= 0); !(gamma > 1); backward not 0/1;
+ *   address ranges of input / output / optional outputs / scratch that intersect       -> GAMER_EINVAL
  *   n_groups == 0                                                     -> GAMER_OK, nothing enqueued
  *   a CUDA runtime error (launch, attribute, copy)                    -> GAMER_ECUDA
  *   an allocation failure inside gamer_hydro_pipeline_run             -> GAMER_ENOMEM
@@ -108,18 +110,22 @@ GAMER_API int gamer_hydro_pipeline_release(void);
 GAMER_API int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int gy, int gz,
                            int bc_x, int bc_y, int bc_z, void* stream);
 
-/* NEXT-3 — multi-step driver on such a box, entirely on the device (no host round trip between steps).  Each of the
- * n_steps steps does: dt = cfl * dh / max over ALL padded cells of (c_s + max_i |v_i|) (Eq.30; fp32,
- * DESIGN.md reading R10); one forward pass d_padded -> d_interior with that dt (read from device memory, constants
- * formed exactly as on the host); gamer_hydro_ghost_fill(d_interior -> d_padded).  The maximum is taken in one pass
- * over the initial state; from then on it is the maximum of the per-group speeds of the updated interiors that the
- * hydro kernel writes as a by-product (:426: "a single floating-point value per patch group") and of the ghost cells
- * beyond "keep" ends, which never change — the same set of cells.  On return (asynchronous on `stream`) d_padded holds
- * the ghost-filled state after n_steps and d_interior its interiors.
+/* NEXT-3 — multi-step driver on such a box, entirely on the device (no host round trip between steps).
+ * order = 0: each of the n_steps steps does: dt = cfl * dh / max over ALL padded cells of (c_s + max_i |v_i|) (Eq.30,
+ *   PAPER.md:418-426; fp32, reading R10); one forward pass d_padded -> d_interior with that dt (read from
+ *   device memory, constants formed exactly as on the host); gamer_hydro_ghost_fill(d_interior -> d_padded).
+ * order = 1: the paper's full step ("a forward sweep in the order xyz, and follows a backward sweep
+ *   in the order zyx.  The same time step must be employed by these two sweeps to maintain the second-order
+ *   accuracy"): dt as above; forward pass; ghost fill; backward pass (z,y,x) with the SAME dt; ghost fill.  A step
+ *   advances the state by 2 dt, and the next dt is evaluated after the backward sweep (:424).
+ * The maximum is taken in one pass over the initial state; from then on it is the maximum of the per-group speeds of
+ * the updated interiors that the last pass of a step writes as a by-product (:426: "a single floating-point value per
+ * patch group") and of the ghost cells beyond "keep" ends, which never change — the same set of cells.  On return
+ * (asynchronous on `stream`) d_padded holds the ghost-filled state after n_steps and d_interior its interiors.
  * d_work: 4 + gx*gy*gz floats of device scratch, 16-byte aligned.  d_dt_log: optional device array of n_steps floats
- * that receives the dt of every step (NULL = off). */
+ * that receives the dt of every step (NULL = off).  order other than 0/1, n_steps < 0, !(cfl > 0) -> GAMER_EINVAL. */
 GAMER_API int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, int gz,
-                            int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dh, float gamma,
+                            int bc_x, int bc_y, int bc_z, int n_steps, int order, float cfl, float dh, float gamma,
                             float* d_work, float* d_dt_log, void* stream);
 
 /* NEXT-4 — one pass in DOUBLE precision (the paper switches to double for its convergence tests).

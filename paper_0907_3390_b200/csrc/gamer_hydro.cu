@@ -28,6 +28,13 @@ int fail(int code, const char* fmt, ...) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// do [a, a + a_bytes) and [b, b + b_bytes) intersect?  (NULL or empty ranges never do)
+bool ranges_overlap(const void* a, size_t a_bytes, const void* b, size_t b_bytes) {
+    if (a == nullptr || b == nullptr || a_bytes == 0 || b_bytes == 0) return false;
+    const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), b0 = reinterpret_cast<uintptr_t>(b);
+    return a0 < b0 + b_bytes && b0 < a0 + a_bytes;
+}
+
 using KernelFn = void (*)(const float*, float*, long long, gamer::GasConst, float*, float*, const float*);
 
 KernelFn pick_kernel(bool backward, bool face, bool speed) {
@@ -61,7 +68,7 @@ struct Staging {
     size_t in_bytes[16] = {};
     size_t out_bytes[16] = {};
 };
-std::mutex g_pipe_mu;
+std::mutex g_pipe_mu[64];      // one per device: calls on different devices do not serialise
 Staging g_staging[64];
 
 // SM count of the current device and the opt-in to 208 KB of dynamic shared memory, once per device and kernel.
@@ -110,6 +117,16 @@ int validate(const void* in, const void* out, long long n_groups, int ghost, flo
     return GAMER_OK;
 }
 
+// The kernel streams results of finished groups to the outputs while later groups are still being read: an output
+// that overlaps the input (or another output) would be corrupted silently.  bytes[i] = extent of ptr[i].
+int check_disjoint(const void* const* ptr, const size_t* bytes, int n) {
+    for (int i = 0; i < n; ++i)
+        for (int j = i + 1; j < n; ++j)
+            if (ranges_overlap(ptr[i], bytes[i], ptr[j], bytes[j]))
+                return fail(GAMER_EINVAL, "input, output and scratch buffers must not overlap");
+    return GAMER_OK;
+}
+
 gamer::GasConst make_const(float dt, float dh, float gamma) {
     gamer::GasConst gc;
     const float k = dt / dh;
@@ -145,8 +162,16 @@ extern "C" {
 
 int gamer_hydro_advance_ex(const float* d_in, float* d_out, long long n_groups, int ghost, float dt, float dh,
                            float gamma, int backward, float* d_face_flux, float* d_group_maxspeed, void* stream) {
-    const int rc = validate(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward, d_face_flux, d_group_maxspeed);
+    int rc = validate(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward, d_face_flux, d_group_maxspeed);
     if (rc != GAMER_OK) return rc;
+    {
+        const size_t n = (size_t)n_groups, fl = sizeof(float);
+        const void* ptr[4] = {d_in, d_out, d_face_flux, d_group_maxspeed};
+        const size_t bytes[4] = {n * gamer::GROUP_IN_FLOATS * fl, n * gamer::GROUP_OUT_FLOATS * fl,
+                                 n * gamer::GROUP_FACE_FLOATS * fl, n * fl};
+        rc = check_disjoint(ptr, bytes, 4);
+        if (rc != GAMER_OK) return rc;
+    }
     g_err[0] = '\0';
     if (n_groups == 0) return GAMER_OK;
     return launch(d_in, d_out, n_groups, dt, dh, gamma, backward, d_face_flux, d_group_maxspeed,
@@ -172,8 +197,15 @@ size_t gamer_hydro_face_flux_floats(long long n_groups) {
 
 int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups, int ghost, float dt, float dh,
                              float gamma, int backward, long long groups_per_chunk, int n_streams) {
-    const int rc = validate(h_in, h_out, n_groups, ghost, dt, dh, gamma, backward, nullptr, nullptr);
+    int rc = validate(h_in, h_out, n_groups, ghost, dt, dh, gamma, backward, nullptr, nullptr);
     if (rc != GAMER_OK) return rc;
+    {
+        const void* ptr[2] = {h_in, h_out};
+        const size_t bytes[2] = {(size_t)n_groups * gamer::GROUP_IN_FLOATS * sizeof(float),
+                                 (size_t)n_groups * gamer::GROUP_OUT_FLOATS * sizeof(float)};
+        rc = check_disjoint(ptr, bytes, 2);
+        if (rc != GAMER_OK) return rc;
+    }
     if (n_streams < 1 || n_streams > 16) return fail(GAMER_EINVAL, "n_streams must be in 1..16");
     if (groups_per_chunk < 1) return fail(GAMER_EINVAL, "groups_per_chunk must be >= 1");
     g_err[0] = '\0';
@@ -188,8 +220,8 @@ int gamer_hydro_pipeline_run(const float* h_in, float* h_out, long long n_groups
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess || dev < 0 || dev >= 64) return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
     // The streams and staging buffers are kept between calls (allocating 3 x 150 MB costs ~10 % of a config-5 call)
-    // and grown when a call needs more; gamer_hydro_pipeline_release() frees them.  Calls are serialised per process.
-    std::lock_guard<std::mutex> lk(g_pipe_mu);
+    // and grown when a call needs more; gamer_hydro_pipeline_release() frees them.  Calls are serialised per device.
+    std::lock_guard<std::mutex> lk(g_pipe_mu[dev]);
     Staging& st = g_staging[dev];
     int status = GAMER_OK;
     for (int s = 0; s < n_streams && status == GAMER_OK; ++s) {
@@ -246,7 +278,7 @@ int gamer_hydro_pipeline_release(void) {
     int dev = 0;
     const cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess || dev < 0 || dev >= 64) return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
-    std::lock_guard<std::mutex> lk(g_pipe_mu);
+    std::lock_guard<std::mutex> lk(g_pipe_mu[dev]);
     Staging& st = g_staging[dev];
     for (int s = 0; s < 16; ++s) {
         if (st.stream[s]) cudaStreamSynchronize(st.stream[s]);
@@ -282,7 +314,7 @@ int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int
 }
 
 int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, int gz, int bc_x, int bc_y, int bc_z,
-                            int n_steps, float cfl, float dh, float gamma, float* d_work, float* d_dt_log,
+                            int n_steps, int order, float cfl, float dh, float gamma, float* d_work, float* d_dt_log,
                             void* stream_) {
     int rc = check_box(gx, gy, gz, bc_x, bc_y, bc_z);
     if (rc != GAMER_OK) return rc;
@@ -291,15 +323,29 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     if (rc != GAMER_OK) return rc;
     if (d_work == nullptr) return fail(GAMER_EINVAL, "d_work must point to 4 + n_groups floats of device memory");
     if (n_steps < 0 || !(cfl > 0.f)) return fail(GAMER_EINVAL, "n_steps must be >= 0 and cfl > 0");
+    if (order != 0 && order != 1) return fail(GAMER_EINVAL, "order must be 0 (forward passes) or 1 (forward + backward pairs)");
+    {
+        const size_t fl = sizeof(float);
+        const void* ptr[4] = {d_padded, d_interior, d_work, d_dt_log};
+        const size_t bytes[4] = {(size_t)n * gamer::GROUP_IN_FLOATS * fl, (size_t)n * gamer::GROUP_OUT_FLOATS * fl,
+                                 (size_t)(4 + n) * fl, (size_t)n_steps * fl};
+        rc = check_disjoint(ptr, bytes, 4);
+        if (rc != GAMER_OK) return rc;
+    }
     g_err[0] = '\0';
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     using namespace gamer;
-    KernelFn fn = hydro_advance_kernel<false, false, true, true>;       // forward, fused CFL speed, dt from the device
+    // dt is read from device memory by every pass; the per-group CFL speed comes out of the LAST pass of a step
+    // ("we can calculate the CFL condition in GPU after the backward sweep")
+    KernelFn fwd = order == 0 ? hydro_advance_kernel<false, false, true, true> : hydro_advance_kernel<false, false, false, true>;
+    KernelFn bwd = hydro_advance_kernel<true, false, true, true>;
     int sm_count = 0;
-    rc = prepare(reinterpret_cast<const void*>(fn), 8, SMEM_BYTES, &sm_count);
+    rc = prepare(reinterpret_cast<const void*>(fwd), order == 0 ? 8 : 11, SMEM_BYTES, &sm_count);
+    if (rc == GAMER_OK && order == 1) rc = prepare(reinterpret_cast<const void*>(bwd), 12, SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
     const int grid = (int)(n < (long long)sm_count ? n : (long long)sm_count);
     const int red_grid = (int)(n < 4ll * sm_count ? n : 4ll * sm_count);
+    const unsigned int gsm_grid = (unsigned int)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024);
     BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
     unsigned int* acc = reinterpret_cast<unsigned int*>(d_work);
     float* d_speed = d_work + 4;
@@ -311,11 +357,16 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
         if (bc_x | bc_y | bc_z) max_speed_kernel<<<red_grid, 256, 0, stream>>>(d_padded, n, gamma, acc + 2, geo, 1);
         max_speed_kernel<<<red_grid, 256, 0, stream>>>(d_padded, n, gamma, acc, geo, 0);
     }
+    const GasConst gc = make_const(0.f, dh, gamma);
     for (int s = 0; s < n_steps && e == cudaSuccess; ++s) {
         cfl_dt_kernel<<<1, 1, 0, stream>>>(d_work, cfl, dh, d_dt_log ? d_dt_log + s : nullptr);
-        fn<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, make_const(0.f, dh, gamma), nullptr,
-                                                        d_speed, d_work + 1);
-        group_speed_max_kernel<<<(unsigned int)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024), 256, 0, stream>>>(d_speed, n, acc);
+        fwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr,
+                                                         order == 0 ? d_speed : nullptr, d_work + 1);
+        if (order == 1) {       // the backward sweep z,y,x follows with the SAME time step
+            ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
+            bwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr, d_speed, d_work + 1);
+        }
+        group_speed_max_kernel<<<gsm_grid, 256, 0, stream>>>(d_speed, n, acc);
         ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
         e = cudaGetLastError();
     }
@@ -345,6 +396,13 @@ int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_group
         return fail(GAMER_EINVAL, "NULL input, output or scratch pointer");
     if (!aligned16(d_in) || !aligned16(d_out) || !aligned16(d_scratch))
         return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
+    {
+        const void* ptr[2] = {d_in, d_out};
+        const size_t bytes[2] = {(size_t)n_groups * gamer::GROUP_IN_FLOATS * sizeof(double),
+                                 (size_t)n_groups * gamer::GROUP_OUT_FLOATS * sizeof(double)};
+        const int rc0 = check_disjoint(ptr, bytes, 2);
+        if (rc0 != GAMER_OK) return rc0;
+    }
     g_err[0] = '\0';
     if (n_groups == 0) return GAMER_OK;
     int sm_count = 0;
@@ -387,13 +445,6 @@ int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem
     g_err[0] = '\0';
     return GAMER_OK;
 }
-
-#ifdef GAMER_PHASE_TIMERS
-// debug builds only (never defined by build.py): per-CTA cycles {wait for planes, x, y, z} of the last launch
-GAMER_API int gamer_debug_phase_cycles(long long* host, int n_ctas) {
-    return (int)cudaMemcpyFromSymbol(host, gamer::g_phase_cycles, sizeof(long long) * 16 * 8 * (size_t)n_ctas);
-}
-#endif
 
 const char* gamer_last_error(void) { return g_err; }
 const char* gamer_version(void) { return "gamer-hydro-b200 0.1.0 (sm_100a)"; }

@@ -26,11 +26,6 @@ constexpr int VAR_FLOATS = NP * NP * NP;                  // 10 648
 constexpr int CTL_BYTES = 512;                            // mbarriers, counters, reduction scratch (struct Ctl)
 constexpr int SMEM_BYTES = GROUP_IN_BYTES + CTL_BYTES;
 
-#ifdef GAMER_PHASE_TIMERS
-// debug builds only (never defined by build.py): per-CTA cycles spent waiting for the load / in each sweep
-__device__ long long g_phase_cycles[160 * 16 * 8];   // [cta][warp][slot]
-#endif
-
 // ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -409,14 +404,6 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
     }
     __syncthreads();
 
-#ifdef GAMER_PHASE_TIMERS
-    long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tt0, tt1;
-#define PHASE_T0() tt0 = clock64()
-#define PHASE_ACC(i) do { tt1 = clock64(); tacc[i] += tt1 - tt0; tt0 = tt1; } while (0)
-#else
-#define PHASE_T0()
-#define PHASE_ACC(i)
-#endif
     NoGate nogate;
     unsigned int it = 0;
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x, ++it) {
@@ -424,7 +411,6 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
         float* out_g = out + g * (long long)GROUP_OUT_FLOATS;
         float* face_g = WANT_FACE ? face_flux + g * (long long)GROUP_FACE_FLOATS : nullptr;
         float speed = 0.f;
-        PHASE_T0();
         if (!BACKWARD) {
             // x sweep: warp w takes the (z,y) rows 32w..32w+31 and starts as soon as their planes have landed.  Warps
             // 8..15 have no z rows and arrive here while the z sweep of the previous group is still running.
@@ -436,15 +422,10 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
                 for (int c = xtask_chunk_lo(warp); c <= xtask_chunk_hi(warp); ++c)
                     named_bar_sync(BAR_FULL + c, full_threads(c));
             }
-            PHASE_ACC(0);
             sweep<0, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, row_lo + lane, nogate);
-            PHASE_ACC(1);
             __syncthreads();
-            PHASE_ACC(4);
             sweep<1, NG, PS, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
-            PHASE_ACC(2);
             __syncthreads();
-            PHASE_ACC(5);
             const long long gn = g + gridDim.x;
             if (warp < N_ZWARP) {
                 ZPlaneGate gate;
@@ -455,7 +436,6 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             } else if (warp == LOADER_WARP && gn < n_groups) {
                 load_next_group(smem, ctl, in + gn * (long long)GROUP_IN_FLOATS);
             }
-            PHASE_ACC(3);
             // no CTA-wide barrier: a plane is overwritten only after all z threads have read it (BAR_ZFREE), and the
             // next group's x tasks wait for their planes (BAR_FULL)
         } else {
@@ -471,13 +451,10 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             ChunkWaitGate zgate;
             zgate.ctl = ctl;
             zgate.parity = parity;
-            PHASE_ACC(0);
             sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, zgate);
             __syncthreads();
-            PHASE_ACC(1);
             sweep<1, 0, NP, NG, PS, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
-            PHASE_ACC(2);
             sweep<0, NG, PS, NG, PS, true, false, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
                                                                          nogate);
             if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);
@@ -491,13 +468,8 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
                 reinterpret_cast<float4*>(out_g)[i] = val;
             }
             __syncthreads();          // every thread is done with the buffer before the next bulk copy overwrites it
-            PHASE_ACC(3);
         }
     }
-#ifdef GAMER_PHASE_TIMERS
-    if (lane == 0)
-        for (int i = 0; i < 8; ++i) g_phase_cycles[(blockIdx.x * 16 + warp) * 8 + i] = tacc[i];
-#endif
 }
 
 }  // namespace gamer

@@ -50,7 +50,7 @@ def lib():
         L.gamer_hydro_ghost_fill.restype = ci
         L.gamer_hydro_ghost_fill.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, vp]
         L.gamer_hydro_run_uniform.restype = ci
-        L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
+        L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
         L.gamer_hydro_advance_f64.restype = ci
         L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp]
         L.gamer_hydro_f64_scratch_doubles.restype = ctypes.c_size_t
@@ -156,11 +156,12 @@ def gamer_hydro_ghost_fill(d_interior, d_padded, gx, gy, gz, bc_x=0, bc_y=0, bc_
     return rc
 
 
-def gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, n_steps, cfl, dh, gamma, d_work,
+def gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, n_steps, order, cfl, dh, gamma, d_work,
                             d_dt_log=None, stream=None, check=True):
-    """n_steps of {CFL dt on the device, forward pass, ghost fill} without leaving the device."""
-    rc = lib().gamer_hydro_run_uniform(_ptr(d_padded), _ptr(d_interior), gx, gy, gz, bc_x, bc_y, bc_z, n_steps, cfl, dh,
-                                       gamma, _ptr(d_work), _ptr(d_dt_log), _stream_ptr(stream))
+    """n_steps of {CFL dt on the device, forward pass, ghost fill [, backward pass with the same dt, ghost fill if
+    order = 1]} without leaving the device."""
+    rc = lib().gamer_hydro_run_uniform(_ptr(d_padded), _ptr(d_interior), gx, gy, gz, bc_x, bc_y, bc_z, n_steps,
+                                       int(order), cfl, dh, gamma, _ptr(d_work), _ptr(d_dt_log), _stream_ptr(stream))
     if check:
         _check(rc)
     return rc

@@ -53,30 +53,64 @@ def test_size_helpers():
     assert "sm_100a" in hydro.gamer_version()
 
 
+def host_buffers():
+    """Disjoint, 16-byte aligned host ranges big enough for ONE group: (keepalive, in, out, face, speed)."""
+    buf = (ctypes.c_float * (53240 + 20480 + 11520 + 64 + 8))()
+    a16 = (ctypes.addressof(buf) + 15) & ~15
+    return buf, a16, a16 + 53240 * 4, a16 + (53240 + 20480) * 4, a16 + (53240 + 20480 + 11520) * 4
+
+
 def test_argument_validation_needs_no_device():
     L = hydro.lib()
-    buf = (ctypes.c_float * 64)()
-    a = ctypes.addressof(buf)
-    a16 = (a + 15) & ~15
+    keep, a_in, a_out, a_face, a_speed = host_buffers()
     # ghost != 3 -> unsupported (7-point stencil, PAPER.md:178)
-    assert L.gamer_hydro_advance(a16, a16, 1, 2, 0.1, 1.0, 1.4, None) == hydro.GAMER_EUNSUPPORTED
+    assert L.gamer_hydro_advance(a_in, a_out, 1, 2, 0.1, 1.0, 1.4, None) == hydro.GAMER_EUNSUPPORTED
     assert "ghost" in hydro.gamer_last_error()
-    assert L.gamer_hydro_advance(a16, a16, -1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance(None, a16, 1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance(a16, a16 + 4, 1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL      # misaligned
-    assert L.gamer_hydro_advance(a16, a16, 1, 3, 0.1, 0.0, 1.4, None) == hydro.GAMER_EINVAL           # dh
-    assert L.gamer_hydro_advance(a16, a16, 1, 3, -0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL          # dt
-    assert L.gamer_hydro_advance(a16, a16, 1, 3, float("nan"), 1.0, 1.4, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance(a16, a16, 1, 3, 0.1, 1.0, 1.0, None) == hydro.GAMER_EINVAL           # gamma
-    assert L.gamer_hydro_advance_ex(a16, a16, 1, 3, 0.1, 1.0, 1.4, 2, None, None, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(a_in, a_out, -1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(None, a_out, 1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(a_in, a_out + 4, 1, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL      # misaligned
+    assert "aligned" in hydro.gamer_last_error()
+    assert L.gamer_hydro_advance(a_in, a_out, 1, 3, 0.1, 0.0, 1.4, None) == hydro.GAMER_EINVAL           # dh
+    assert L.gamer_hydro_advance(a_in, a_out, 1, 3, -0.1, 1.0, 1.4, None) == hydro.GAMER_EINVAL          # dt
+    assert L.gamer_hydro_advance(a_in, a_out, 1, 3, float("nan"), 1.0, 1.4, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance(a_in, a_out, 1, 3, 0.1, 1.0, 1.0, None) == hydro.GAMER_EINVAL           # gamma
+    assert L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 2, None, None, None) == hydro.GAMER_EINVAL
     # n_groups == 0 is a successful no-op, even with NULL buffers
     assert L.gamer_hydro_advance(None, None, 0, 3, 0.1, 1.0, 1.4, None) == hydro.GAMER_OK
     assert hydro.gamer_last_error() == ""
-    assert L.gamer_hydro_pipeline_run(a16, a16, 1, 3, 0.1, 1.0, 1.4, 0, 0, 4) == hydro.GAMER_EINVAL   # chunk
-    assert L.gamer_hydro_pipeline_run(a16, a16, 1, 3, 0.1, 1.0, 1.4, 0, 8, 0) == hydro.GAMER_EINVAL   # streams
+    assert L.gamer_hydro_pipeline_run(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 0, 0, 4) == hydro.GAMER_EINVAL   # chunk
+    assert L.gamer_hydro_pipeline_run(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 0, 8, 0) == hydro.GAMER_EINVAL   # streams
     assert L.gamer_hydro_pipeline_run(None, None, 0, 3, 0.1, 1.0, 1.4, 0, 8, 2) == hydro.GAMER_OK
     with pytest.raises(hydro.GamerError):
-        hydro.gamer_hydro_advance(a16, a16, 1, 4, 0.1, 1.0, 1.4, stream=0)
+        hydro.gamer_hydro_advance(a_in, a_out, 1, 4, 0.1, 1.0, 1.4, stream=0)
+
+
+def test_overlapping_buffers_are_refused_without_a_device():
+    """The header forbids overlap between input, outputs and scratch (results of finished groups are streamed out while
+    later groups are still being read); the address ranges are checked before any CUDA call."""
+    L = hydro.lib()
+    keep, a_in, a_out, a_face, a_speed = host_buffers()
+
+    def refused(rc):
+        return rc == hydro.GAMER_EINVAL and "overlap" in hydro.gamer_last_error()
+
+    assert refused(L.gamer_hydro_advance(a_in, a_in, 1, 3, 0.1, 1.0, 1.4, None))                       # out == in
+    assert refused(L.gamer_hydro_advance(a_in, a_in + 212960 - 16, 1, 3, 0.1, 1.0, 1.4, None))         # last 16 B of in
+    assert refused(L.gamer_hydro_advance(a_in + 81920 - 16, a_in, 1, 3, 0.1, 1.0, 1.4, None))          # in starts in out
+    assert refused(L.gamer_hydro_advance(a_in, a_in + 212960, 2, 3, 0.1, 1.0, 1.4, None))              # 2 groups: in grows
+    assert refused(L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 0, a_out + 81920 - 16, None, None))
+    assert refused(L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 1, a_face, a_face + 16, None))
+    assert refused(L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 1, None, a_in + 64, None))
+    assert refused(L.gamer_hydro_pipeline_run(a_in, a_in + 1024, 1, 3, 0.1, 1.0, 1.4, 0, 8, 2))
+    assert refused(L.gamer_hydro_advance_f64(a_in, a_in + 64, 1, 3, 0.1, 1.0, 1.4, 0, a_out, None))
+    # d_work (4 + n floats) inside the padded array; the dt log inside d_work
+    assert refused(L.gamer_hydro_run_uniform(a_in, a_out, 1, 1, 1, 0, 0, 0, 1, 0, 0.5, 1.0, 1.4, a_in + 160, None, None))
+    assert refused(L.gamer_hydro_run_uniform(a_in, a_out, 1, 1, 1, 0, 0, 0, 4, 1, 0.5, 1.0, 1.4, a_face, a_face + 16, None))
+    # adjacent ranges do not overlap: without a device this call passes validation and fails at the first CUDA call
+    # (with a device it would launch on host pointers, so it is only made where there is none)
+    import torch
+    if not torch.cuda.is_available():
+        assert L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 0, a_face, a_speed, None) == hydro.GAMER_ECUDA
 
 
 def test_oracle_and_product_do_not_import_each_other():

@@ -137,15 +137,19 @@ def test_oracle_run_uniform_is_second_order_with_strang_pairs():
 def test_ghost_fill_argument_validation_needs_no_device():
     import ctypes
     L = hydro.lib()
-    buf = (ctypes.c_float * 64)()
-    a16 = (ctypes.addressof(buf) + 15) & ~15
-    assert L.gamer_hydro_ghost_fill(a16, a16, 0, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_ghost_fill(a16, a16, 1, 1, 1, 2, 0, 0, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_ghost_fill(None, a16, 1, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_ghost_fill(a16, a16 + 4, 1, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_run_uniform(a16, a16, 1, 1, 1, 0, 0, 0, 1, 0.5, 1.0, 1.4, None, None, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_run_uniform(a16, a16, 1, 1, 1, 0, 0, 0, 1, 0.0, 1.0, 1.4, a16, None, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_run_uniform(a16, a16, 1, 1, 1, 0, 0, 0, -1, 0.5, 1.0, 1.4, a16, None, None) == hydro.GAMER_EINVAL
+    buf = (ctypes.c_float * (53240 + 20480 + 64))()
+    pad = (ctypes.addressof(buf) + 15) & ~15
+    inter, work = pad + 53240 * 4, pad + (53240 + 20480) * 4
+    assert L.gamer_hydro_ghost_fill(inter, pad, 0, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_ghost_fill(inter, pad, 1, 1, 1, 2, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_ghost_fill(None, pad, 1, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_ghost_fill(inter, pad + 4, 1, 1, 1, 0, 0, 0, None) == hydro.GAMER_EINVAL
+    ru = L.gamer_hydro_run_uniform
+    assert ru(pad, inter, 1, 1, 1, 0, 0, 0, 1, 0, 0.5, 1.0, 1.4, None, None, None) == hydro.GAMER_EINVAL     # no d_work
+    assert ru(pad, inter, 1, 1, 1, 0, 0, 0, 1, 0, 0.0, 1.0, 1.4, work, None, None) == hydro.GAMER_EINVAL     # cfl
+    assert ru(pad, inter, 1, 1, 1, 0, 0, 0, -1, 0, 0.5, 1.0, 1.4, work, None, None) == hydro.GAMER_EINVAL    # n_steps
+    assert ru(pad, inter, 1, 1, 1, 0, 0, 0, 1, 2, 0.5, 1.0, 1.4, work, None, None) == hydro.GAMER_EINVAL     # order
+    assert "order" in hydro.gamer_last_error()
 
 
 # ---------------------------------------------------------------------------------------------------------- GPU
@@ -183,7 +187,7 @@ def test_gpu_run_uniform_config2_sod(axis):
     d_i = torch.empty((inp.shape[0], 5, 16, 16, 16), dtype=torch.float32, device="cuda")
     d_work = torch.zeros(4 + d_i.shape[0], dtype=torch.float32, device="cuda")
     d_log = torch.zeros(nsteps, dtype=torch.float32, device="cuda")
-    hydro.gamer_hydro_run_uniform(d_p, d_i, gx, gy, gz, bc[0], bc[1], bc[2], nsteps, 0.5, dh, gamma, d_work, d_log)
+    hydro.gamer_hydro_run_uniform(d_p, d_i, gx, gy, gz, bc[0], bc[1], bc[2], nsteps, 0, 0.5, dh, gamma, d_work, d_log)
     torch.cuda.synchronize()
     got, dts = d_p.cpu().numpy(), d_log.cpu().numpy().astype(np.float64)
     # the transverse sweeps are exact no-ops, so the oracle chain can run on one column of groups
@@ -212,7 +216,7 @@ def test_gpu_run_uniform_one_step_equals_advance_plus_ghost_fill():
     d_i = torch.empty((8, 5, 16, 16, 16), dtype=torch.float32, device="cuda")
     d_work = torch.zeros(4 + d_i.shape[0], dtype=torch.float32, device="cuda")
     d_log = torch.zeros(1, dtype=torch.float32, device="cuda")
-    hydro.gamer_hydro_run_uniform(d_p, d_i, 2, 2, 2, 0, 0, 0, 1, 0.5, c["dh"], c["gamma"], d_work, d_log)
+    hydro.gamer_hydro_run_uniform(d_p, d_i, 2, 2, 2, 0, 0, 0, 1, 0, 0.5, c["dh"], c["gamma"], d_work, d_log)
     torch.cuda.synchronize()
     dt = float(d_log.cpu().numpy()[0])
     ref_speed = oracle.max_signal_speed(c["inp"], c["gamma"])
@@ -226,3 +230,74 @@ def test_gpu_run_uniform_one_step_equals_advance_plus_ghost_fill():
     assert torch.equal(d_out.view(torch.int32), d_i.view(torch.int32))
     assert torch.equal(d_p2.view(torch.int32), d_p.view(torch.int32))
     assert np.array_equal(d_p.cpu().numpy(), oracle.ghost_fill(d_i.cpu().numpy(), grid))
+
+
+@pytest.mark.gpu
+def test_gpu_run_uniform_strang_pairs_match_the_oracle_chain():
+    """order = 1: forward pass, ghost fill, backward pass with the SAME dt, ghost fill, on the device.
+    Free-running against the oracle's chain over 3 steps (6 passes) on config 1 as a periodic 2x2x2 box: dt sequence to
+    2e-6, state to 1e-4 (6 passes of <= 1e-5 each, metric R11); and one step must give the same bits as the plain
+    entry points called with the logged dt (teacher-forced: each call <= 1e-5 against the oracle on the same input)."""
+    import torch
+    c = W.config1()
+    grid, n_steps = (2, 2, 2), 3
+    d_p = torch.from_numpy(c["inp"]).cuda()
+    d_i = torch.empty((8, 5, 16, 16, 16), dtype=torch.float32, device="cuda")
+    d_work = torch.zeros(4 + 8, dtype=torch.float32, device="cuda")
+    d_log = torch.zeros(n_steps, dtype=torch.float32, device="cuda")
+    hydro.gamer_hydro_run_uniform(d_p, d_i, 2, 2, 2, 0, 0, 0, n_steps, 1, 0.4, c["dh"], c["gamma"], d_work, d_log)
+    torch.cuda.synchronize()
+    got, dts = d_p.cpu().numpy(), d_log.cpu().numpy().astype(np.float64)
+    ref, ref_dts = oracle.run_uniform(c["inp"], grid, (0, 0, 0), n_steps, 0.4, c["dh"], c["gamma"], n_threads=8, order=1)
+    assert np.max(np.abs(dts - np.array(ref_dts)) / np.array(ref_dts)) <= 2e-6
+    e = W.parity_error(got[:, :, 3:19, 3:19, 3:19], ref[:, :, 3:19, 3:19, 3:19], c["gamma"])
+    assert e["max_rel"] <= 1e-4, e
+    assert np.array_equal(got, oracle.ghost_fill(d_i.cpu().numpy(), grid))
+    # one step, written out with the plain entry points and the dt the driver logged
+    d_p1 = torch.from_numpy(c["inp"]).cuda()
+    hydro.gamer_hydro_run_uniform(d_p1, d_i, 2, 2, 2, 0, 0, 0, 1, 1, 0.4, c["dh"], c["gamma"], d_work, d_log)
+    torch.cuda.synchronize()
+    dt = float(d_log.cpu().numpy()[0])
+    d_in = torch.from_numpy(c["inp"]).cuda()
+    d_out = torch.empty_like(d_i)
+    d_pad = torch.full_like(d_in, float("nan"))
+    hydro.gamer_hydro_advance(d_in, d_out, 8, 3, dt, c["dh"], c["gamma"])
+    fwd = d_out.cpu().numpy()
+    e = W.parity_error(fwd, oracle.hydro_advance(c["inp"], dt, c["dh"], c["gamma"]), c["gamma"])
+    assert e["max_rel"] <= 1e-5, e
+    hydro.gamer_hydro_ghost_fill(d_out, d_pad, 2, 2, 2)
+    mid = d_pad.cpu().numpy()
+    hydro.gamer_hydro_advance_ex(d_pad, d_out, 8, 3, dt, c["dh"], c["gamma"], backward=1)
+    torch.cuda.synchronize()
+    e = W.parity_error(d_out.cpu().numpy(), oracle.hydro_advance(mid, dt, c["dh"], c["gamma"], backward=1), c["gamma"])
+    assert e["max_rel"] <= 1e-5, e
+    assert torch.equal(d_out.view(torch.int32), d_i.view(torch.int32))
+
+
+@pytest.mark.gpu
+def test_gpu_run_uniform_diagonal_sound_wave_converges_with_strang_pairs():
+    """The paper's accuracy test (:450-458) through the device-only driver with order = 1, in single precision: a sound
+    wave of amplitude 1e-3 (well above fp32 round-off, still linear to 1e-3) along the box diagonal for one period on
+    16^3 and 32^3 cells; the L1 error of the density falls faster than first order."""
+    import torch
+    gamma, amp = 5.0 / 3.0, 1e-3
+
+    def run(n):
+        dh = 1.0 / n
+        g = n // 16
+        inp = W.box_to_groups(diagonal_wave(n, 0.0, amp=amp)).astype(np.float32)
+        dt0 = 0.4 * dh / 1.3
+        n_steps = int(round((1.0 / DIAG_SPEED) / (2 * dt0)))
+        d_p = torch.from_numpy(inp).cuda()
+        d_i = torch.empty((g ** 3, 5, 16, 16, 16), dtype=torch.float32, device="cuda")
+        d_work = torch.zeros(4 + g ** 3, dtype=torch.float32, device="cuda")
+        d_log = torch.zeros(n_steps, dtype=torch.float32, device="cuda")
+        hydro.gamer_hydro_run_uniform(d_p, d_i, g, g, g, 0, 0, 0, n_steps, 1, 0.4, dh, gamma, d_work, d_log)
+        torch.cuda.synchronize()
+        t = 2.0 * float(d_log.cpu().numpy().astype(np.float64).sum())
+        box = W.groups_to_box(d_i.cpu().numpy().astype(np.float64), (g, g, g))
+        return np.mean(np.abs(box[0] - diagonal_wave(n, DIAG_SPEED * t, amp=amp)[0])) / amp
+
+    e16, e32 = run(16), run(32)
+    slope = np.log2(e32 / e16)
+    assert -2.6 <= slope <= -1.4, (e16, e32, slope)
