@@ -32,8 +32,9 @@ METRIC = "hydro cell-updates/sec (fp32) on 1 B200; % of roofline (HBM GB/s)"
 UNIT = "cell-updates/s"
 CELLS_PER_GROUP = 16 ** 3
 BYTES_PER_GROUP = 212960 + 81920            # padded in + interior out
-FLOPS_PER_GROUP = 1092 * 3474                # rows x flops per row, FMA = 2
+FLOPS_PER_GROUP = 1092 * 3474                # rows x flops per row, FMA = 2: the SMALLEST count
 FP32_LANES_PER_SM = 128
+PARITY_TOL = 1e-5                            # GPU vs fp32 oracle, metric R11 (north_star)
 
 
 def load_peaks():
@@ -97,20 +98,41 @@ class ClockSampler(threading.Thread):
                     samples=len(self.samples))
 
 
-def profiled_traffic(config, n_groups):
-    """DRAM bytes per launch of the hydro kernel from the committed ncu capture (profiles/), if it matches the workload."""
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) over the CUDA sources of the library, in name order: identifies the kernel build
+    that a profiles/*_traffic.csv row was captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    cdir = os.path.join(ROOT, "paper_0907_3390_b200", "csrc")
+    for fn in sorted(os.listdir(cdir)):
+        if fn.endswith((".cu", ".cuh")):
+            h.update(fn.encode())
+            h.update(open(os.path.join(cdir, fn), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def profiled_traffic(config, n_groups, kernel="forward"):
+    """(DRAM bytes per launch, source tag) of the hydro kernel from a committed ncu capture under profiles/ — only if the
+    row names this workload AND was captured on the current kernel sources (kernel_src_sha16); else (None, why)."""
     import csv
-    best = None
     pdir = os.path.join(ROOT, "profiles")
-    if not os.path.isdir(pdir):
-        return None
-    for fn in sorted(os.listdir(pdir)):
-        if fn.endswith("_traffic.csv"):
+    sha = kernel_source_hash()
+    stale = None
+    if os.path.isdir(pdir):
+        for fn in sorted(os.listdir(pdir), reverse=True):
+            if not fn.endswith("_traffic.csv"):
+                continue
             with open(os.path.join(pdir, fn)) as f:
                 for row in csv.DictReader(f):
-                    if row["workload"] == "config%d" % config and int(row["n_groups"]) == n_groups:
-                        best = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
-    return best
+                    if row.get("workload") != "config%d" % config or int(row["n_groups"]) != n_groups:
+                        continue
+                    if row.get("kernel", "forward") != kernel:
+                        continue
+                    if row.get("kernel_src_sha16") == sha:
+                        return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]), \
+                            "profiles/%s (ncu --set full, kernel sources %s)" % (fn, sha)
+                    stale = "profiles/%s is of kernel sources %s, current %s" % (fn, row.get("kernel_src_sha16"), sha)
+    return None, stale or "no ncu capture of this workload under profiles/"
 
 
 def max_over_ranks(x, dist, device):
@@ -154,6 +176,19 @@ def make_device_workload(config, torch, device, n_override=None):
     inp = c["inp"] if n_override is None else c["inp"][:n_override]
     d_in = torch.from_numpy(inp).to(device)
     return d_in, inp.shape[0], c["dt"], c["dh"], c["gamma"], "%s: %d groups" % (c["name"], inp.shape[0])
+
+
+def time_advance(hydro, torch, stream, d_in, d_out, n, dt, dh, gamma, backward=0, steps=10, warmup=3):
+    """mean ms per launch of one pass over n groups, CUDA events on `stream`."""
+    for _ in range(warmup):
+        hydro.gamer_hydro_advance_ex(d_in, d_out, n, 3, dt, dh, gamma, backward, stream=stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        hydro.gamer_hydro_advance_ex(d_in, d_out, n, 3, dt, dh, gamma, backward, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
 
 
 def cpu_sample(config, n_sample):
@@ -263,8 +298,8 @@ def run_ours(args):
     kernel_ms = float(np.mean(per_launch_ms))
 
     # CPU baseline leg: the oracle as it stands on the host cores, on the first groups of the same workload.  Its
-    # output doubles as a check of the timed output on those groups, so that a wrong-but-fast run cannot pass.
-    cpu_baseline, parity = None, None
+    # output doubles as a check of the timed output on those groups: a wrong-but-fast run makes bench.py exit 1.
+    cpu_baseline, parity, cpu_1thread, failed = None, None, None, []
     if rank == 0 and world == 1 and not args.no_cpu:
         cores = os.cpu_count() or 1
         cpu_baseline, cs, _ = time_oracle(args.config, cores)
@@ -272,6 +307,17 @@ def run_ours(args):
             ns = cs["out"].shape[0]
             parity = W.parity_error(d_out[:ns].cpu().numpy(), cs["out"], gamma)["max_rel"]
             cpu_baseline["parity_max_rel_on_sample"] = parity
+            if not parity <= PARITY_TOL:
+                failed.append("parity on the first %d groups: %.3g > %.0e" % (ns, parity, PARITY_TOL))
+        # the plain oracle, fp32, ONE thread, on config 3 (512 groups)
+        import oracle
+        c3 = W.config3()
+        t0 = time.perf_counter()
+        oracle.hydro_advance(c3["inp"], c3["dt"], c3["dh"], c3["gamma"], n_threads=1)
+        w3 = time.perf_counter() - t0
+        cpu_1thread = dict(value=c3["inp"].shape[0] * CELLS_PER_GROUP / w3, unit=UNIT, cores=1, kind="oracle",
+                           sample="config3, all %d groups, fp32 oracle, 1 thread, %.2f s wall" % (c3["inp"].shape[0], w3))
+        del c3
 
     # roofline of the one kernel of the step
     n_sm = torch.cuda.get_device_properties(device).multi_processor_count
@@ -281,18 +327,69 @@ def run_ours(args):
     roofline_hbm = dict(bound="hbm", achieved=ach_gbs, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach_gbs / peaks["hbm_gbs"],
                         traffic=None, peak_source=peaks["source"])
     roofline_alu = dict(bound="alu", achieved=ach_tf, peak=fp32_peak_tflops, unit="TFLOP/s", frac=ach_tf / fp32_peak_tflops,
-                        traffic=None, peak_source="derived: %d SM x 128 FP32 lanes x 2 x sm_max_mhz (DESIGN.md)" % n_sm)
+                        traffic=None, peak_source="derived: %d SM x 128 FP32 lanes x 2 x sm_max_mhz (DESIGN.md); `frac` "
+                                                  "uses this one, the measured FMA rate is beside it" % n_sm)
+    # the FMA-only micro-benchmark of the library, measured in this run
+    d_sink = torch.zeros(4, dtype=torch.float32, device=device)
+    peak_meas_tf, peak_meas_lanes = hydro.gamer_hydro_fp32_peak(5, d_sink, peaks["sm_max_mhz"])
+    roofline_alu["peak_measured_tflops"] = peak_meas_tf
+    roofline_alu["peak_measured_fma_per_clk_per_sm"] = peak_meas_lanes
+    roofline_alu["frac_of_measured_peak"] = ach_tf / peak_meas_tf
     # the metric's roofline is the slower of the two bounds (north_star): FP32 at 51 ns/group vs HBM at 45 ns/group
     t_alu = FLOPS_PER_GROUP / (fp32_peak_tflops * 1e12)
     t_hbm = BYTES_PER_GROUP / (peaks["hbm_gbs"] * 1e9)
     roofline = dict(roofline_alu if t_alu >= t_hbm else roofline_hbm)
-    traffic = profiled_traffic(args.config, n)
+    traffic, traffic_source = profiled_traffic(args.config, n)
     for r in (roofline, roofline_hbm, roofline_alu):
         r["traffic"] = traffic
+        r["traffic_source"] = traffic_source
     roofline["algorithmic_bytes"] = n * BYTES_PER_GROUP
     roofline["algorithmic_flops"] = n * FLOPS_PER_GROUP
+    roofline["flops_per_group"] = FLOPS_PER_GROUP
+    roofline["flops_count"] = ("hand count 1092 rows x 3474 (SURVEY 8(d)), the smallest of three: the kernel's own "
+                               "formulation is 3492 per row, the oracle's literal Eq.8 counts 5.33 M per group")
     roofline["kernel_ms"] = kernel_ms
     roofline["ns_per_group"] = kernel_ms * 1e6 / n
+
+    # fp32 backward pass (z,y,x), same workload: half of every forward+backward step of the paper (:174-176)
+    backward = None
+    if rank == 0:
+        ms_b = time_advance(hydro, torch, stream, d_in, d_out, n, dt, dh, gamma, backward=1, steps=10)
+        backward = dict(ns_per_group=ms_b * 1e6 / n, ratio_to_forward=ms_b / kernel_ms,
+                        frac=(n * FLOPS_PER_GROUP / (ms_b * 1e-3) / 1e12) / fp32_peak_tflops)
+        hydro.gamer_hydro_advance(d_in, d_out, n, 3, dt, dh, gamma, stream=stream)      # d_out = the forward result again
+        torch.cuda.synchronize()
+
+    # config 4 (the arithmetic-realistic input): as specified (4096 groups) and tiled to 32 768 groups
+    config4 = None
+    if rank == 0 and world == 1 and args.config == 5 and not args.no_config4:
+        c4 = W.config4()
+        n4 = c4["inp"].shape[0]
+        d4 = torch.from_numpy(c4["inp"]).to(device)
+        o4 = torch.empty((n4, 5, 16, 16, 16), dtype=torch.float32, device=device)
+        ms4 = time_advance(hydro, torch, stream, d4, o4, n4, c4["dt"], c4["dh"], c4["gamma"], steps=20)
+        config4 = dict(workload="config4: %d groups (lognormal density, sigma(ln rho) = 2, reading R17)" % n4,
+                       n_groups=n4, ns_per_group=ms4 * 1e6 / n4,
+                       frac=(n4 * FLOPS_PER_GROUP / (ms4 * 1e-3) / 1e12) / fp32_peak_tflops)
+        if not args.no_cpu and not args.no_check:
+            import oracle
+            ns4 = 512
+            ref4 = oracle.hydro_advance(c4["inp"][:ns4], c4["dt"], c4["dh"], c4["gamma"], n_threads=os.cpu_count() or 1)
+            p4 = W.parity_error(o4[:ns4].cpu().numpy(), ref4, c4["gamma"])["max_rel"]
+            config4["parity_max_rel_on_first_%d_groups" % ns4] = p4
+            if not p4 <= PARITY_TOL:
+                failed.append("config 4 parity: %.3g > %.0e" % (p4, PARITY_TOL))
+        rep = n // n4
+        if rep > 1 and n4 * rep * (BYTES_PER_GROUP) < 12e9:
+            d4r = d4.repeat(rep, 1, 1, 1, 1)
+            o4r = torch.empty((n4 * rep, 5, 16, 16, 16), dtype=torch.float32, device=device)
+            ms4r = time_advance(hydro, torch, stream, d4r, o4r, n4 * rep, c4["dt"], c4["dh"], c4["gamma"], steps=10)
+            config4["tiled_x%d" % rep] = dict(n_groups=n4 * rep, ns_per_group=ms4r * 1e6 / (n4 * rep),
+                                              frac=(n4 * rep * FLOPS_PER_GROUP / (ms4r * 1e-3) / 1e12) / fp32_peak_tflops,
+                                              ratio_to_config5=(ms4r / (n4 * rep)) / (kernel_ms / n))
+            del d4r, o4r
+        del d4, o4, c4
+        torch.cuda.empty_cache()
 
     # end to end through the public C-ABI call with host buffers
     e2e = None
@@ -416,12 +513,16 @@ def run_ours(args):
                                 l2="inputs (%.2f GB) larger than L2; no flush needed" % (d_in.numel() * 4 / 1e9),
                                 launch=info),
                     roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
-                    cpu_baseline=cpu_baseline, e2e=e2e, gpu_launches=args.steps, clocks=clocks,
+                    cpu_baseline=cpu_baseline, cpu_baseline_1thread=cpu_1thread, e2e=e2e, gpu_launches=args.steps,
+                    clocks=clocks, backward=backward, config4=config4, failed=failed,
                     next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs, next4_f64=f64, next3_run_uniform=run_uniform,
                     parity_spot_check_max_rel=parity)
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+    if failed:
+        print("bench.py: FAILED: " + "; ".join(failed), file=sys.stderr)
+        return 1
     return 0
 
 
@@ -439,6 +540,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
     ap.add_argument("--no-check", action="store_true")
+    ap.add_argument("--no-config4", action="store_true", help="skip the config-4 sub-record")
     ap.add_argument("--no-ghost-fill", action="store_true", help="skip the separate ghost-fill measurement")
     args = ap.parse_args()
     if args.impl == "reference":

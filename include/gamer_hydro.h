@@ -145,6 +145,15 @@ GAMER_API size_t gamer_hydro_f64_scratch_doubles(void);
  * bytes, regs = registers per thread of the kernel. */
 GAMER_API int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread);
 
+/* Measurement aid for the roofline: an FMA-only micro-benchmark of the FP32 pipe of the current
+ * device — 4 CTAs of 512 threads per SM, 16 independent fused multiply-add chains per thread, 2048 steps each —
+ * launched repeats + 1 times on the default stream (the first is a warm-up), timed with CUDA events; SYNCHRONOUS.
+ * *tflops receives the best launch's 2 x FMA count / time in TFLOP/s; *lane_fma_per_clk_per_sm (optional) the same as
+ * FMAs per clock per SM if sm_mhz (the SM clock the caller observed, MHz) is > 0 — 128 is the unit count of the part.
+ * d_sink: one float of device memory (never written in practice).  Not part of the hydro path. */
+GAMER_API int gamer_hydro_fp32_peak(int repeats, float* d_sink, double* tflops, double* lane_fma_per_clk_per_sm,
+                          double sm_mhz);
+
 GAMER_API const char* gamer_last_error(void);   /* thread-local, static storage; "" if the last call on this thread succeeded */
 GAMER_API const char* gamer_version(void);      /* static string */
 

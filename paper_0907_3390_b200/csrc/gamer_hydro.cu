@@ -156,6 +156,25 @@ int launch(const float* d_in, float* d_out, long long n_groups, float dt, float 
     return GAMER_OK;
 }
 
+// FMA-only micro-benchmark of the FP32 pipe ("measures an FMA-only micro-benchmark, and states which
+// number is used"): 16 independent FFMA chains per thread, nothing else in the loop but its counter.
+constexpr int PEAK_CHAINS = 16, PEAK_ITERS = 2048, PEAK_THREADS = 512, PEAK_CTAS_PER_SM = 4;
+__global__ void __launch_bounds__(PEAK_THREADS) fp32_peak_kernel(float* __restrict__ sink, float a, float b) {
+    float x[PEAK_CHAINS];
+#pragma unroll
+    for (int i = 0; i < PEAK_CHAINS; ++i) x[i] = 1e-3f * (float)(threadIdx.x + i);
+    const float m = a + 1e-9f * (float)(threadIdx.x & 1), c = b;      // per-thread values: stay in vector registers
+#pragma unroll 8
+    for (int it = 0; it < PEAK_ITERS; ++it) {
+#pragma unroll
+        for (int i = 0; i < PEAK_CHAINS; ++i) x[i] = fmaf(x[i], m, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < PEAK_CHAINS; ++i) s += x[i];
+    if (s == 123.456f) sink[0] = s;                                    // keeps the chains alive, never true in practice
+}
+
 }  // namespace
 
 extern "C" {
@@ -442,6 +461,35 @@ int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem
     if (block) *block = gamer::BLOCK_THREADS;
     if (smem_bytes) *smem_bytes = smem;
     if (regs_per_thread) *regs_per_thread = fa.numRegs;
+    g_err[0] = '\0';
+    return GAMER_OK;
+}
+
+int gamer_hydro_fp32_peak(int repeats, float* d_sink, double* tflops, double* lane_fma_per_clk_per_sm, double sm_mhz) {
+    if (repeats < 1 || d_sink == nullptr || tflops == nullptr) return fail(GAMER_EINVAL, "repeats >= 1, d_sink and tflops non-NULL");
+    int dev = 0, sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(GAMER_ECUDA, "no CUDA device: %s", cudaGetErrorString(e)); }
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(GAMER_ECUDA, "cudaEventCreate");
+    const int grid = sm * PEAK_CTAS_PER_SM;
+    double best_ms = 1e30;
+    for (int r = 0; r < repeats + 1 && e == cudaSuccess; ++r) {           // the first launch is a warm-up
+        cudaEventRecord(e0, 0);
+        fp32_peak_kernel<<<grid, PEAK_THREADS>>>(d_sink, 1.0000001f, 1e-7f);
+        cudaEventRecord(e1, 0);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess) return fail(GAMER_ECUDA, "fp32_peak: %s", cudaGetErrorString(e));
+    const double fma = (double)grid * PEAK_THREADS * PEAK_CHAINS * PEAK_ITERS;
+    *tflops = 2.0 * fma / (best_ms * 1e-3) / 1e12;
+    if (lane_fma_per_clk_per_sm) *lane_fma_per_clk_per_sm = sm_mhz > 0 ? fma / (best_ms * 1e-3) / (sm_mhz * 1e6) / sm : 0.0;
     g_err[0] = '\0';
     return GAMER_OK;
 }

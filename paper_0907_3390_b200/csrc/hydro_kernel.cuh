@@ -70,7 +70,7 @@ struct SmemSink {
     float held[NCOMP];
     template <int ODD>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
-        if (STRIDE == 1) {
+        if (STRIDE == 1 && !GAMER_X32) {
             if (ODD) {
                 if (j == NG) {
 #pragma unroll
@@ -117,7 +117,7 @@ struct FinalSink {
         if (TO_GLOBAL) {
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) dst[k][(j - NG) * OSTRIDE] = u[k];
-        } else if (STRIDE == 1) {
+        } else if (STRIDE == 1 && !GAMER_X32) {
             if (ODD) {
                 if (j == NG) {
 #pragma unroll

@@ -22,6 +22,10 @@
 #define GAMER_MARCH_UNROLL 3     /* pairs of cells per loop body (measured: 1: 113.5, 2: 105.4, 3: 104.5, 4: 108.4 ns/group) */
 #endif
 
+#ifndef GAMER_X32
+#define GAMER_X32 0       /* experiment: 32-bit shared-memory accesses along x */
+#endif
+
 #ifndef GAMER_MARCH_UNROLL_F64
 #define GAMER_MARCH_UNROLL_F64 1
 #endif
@@ -305,7 +309,7 @@ template <int STRIDE>
 struct StrideSrc {
     const float* src[NCOMP];
     __device__ __forceinline__ void load(int n, float (&ua)[NCOMP], float (&ub)[NCOMP]) const {
-        if (STRIDE == 1) {
+        if (STRIDE == 1 && !GAMER_X32) {
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) {
                 const float2 t = *reinterpret_cast<const float2*>(src[k] + n);

@@ -57,6 +57,9 @@ def lib():
         L.gamer_hydro_f64_scratch_doubles.argtypes = []
         L.gamer_hydro_launch_info.restype = ci
         L.gamer_hydro_launch_info.argtypes = [ll] + [ctypes.POINTER(ci)] * 4
+        L.gamer_hydro_fp32_peak.restype = ci
+        L.gamer_hydro_fp32_peak.argtypes = [ci, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                            ctypes.c_double]
         L.gamer_last_error.restype = ctypes.c_char_p
         L.gamer_last_error.argtypes = []
         L.gamer_version.restype = ctypes.c_char_p
@@ -179,6 +182,13 @@ def gamer_hydro_advance_f64(d_in, d_out, n_groups, ghost, dt, dh, gamma, d_scrat
     if check:
         _check(rc)
     return rc
+
+
+def gamer_hydro_fp32_peak(repeats, d_sink, sm_mhz=0.0):
+    """FMA-only micro-benchmark of the FP32 pipe (measurement aid): returns (TFLOP/s, FMAs per clock per SM)."""
+    t, l = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().gamer_hydro_fp32_peak(int(repeats), _ptr(d_sink), ctypes.byref(t), ctypes.byref(l), float(sm_mhz)))
+    return t.value, l.value
 
 
 def gamer_hydro_launch_info(n_groups):

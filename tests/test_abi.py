@@ -28,7 +28,7 @@ def test_header_declares_the_survey_entry_points():
               # beyond the survey's list: NEXT-2 size helper, NEXT-3, NEXT-4, pipeline housekeeping, reporting
               "gamer_hydro_face_flux_floats", "gamer_hydro_ghost_fill", "gamer_hydro_run_uniform",
               "gamer_hydro_advance_f64", "gamer_hydro_f64_scratch_doubles", "gamer_hydro_pipeline_release",
-              "gamer_hydro_launch_info"):
+              "gamer_hydro_launch_info", "gamer_hydro_fp32_peak"):
         assert s in syms
 
 
