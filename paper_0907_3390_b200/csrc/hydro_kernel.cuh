@@ -104,7 +104,10 @@ struct SmemSink {
 
 // Writes the updated cells of the LAST sweep.  TO_GLOBAL: straight to out[g][v][.][.][.] with element stride OSTRIDE
 // along the row; else in place in shared memory.  Tracks the CFL speed of the updated cells if WANT_SPEED.
-template <int STRIDE, int OSTRIDE, bool TO_GLOBAL, bool WANT_SPEED>
+// ALIGNED (backward pass, x sweep in place): the 16 new cells of a row are written 3 (even y) or 1 (odd y) cells to the
+// left of where they belong, i.e. starting on a 16-byte boundary of shared memory, so that the copy-out reads them
+// with 128-bit loads; dst[] already carries that shift.  Safe in place: the march never re-reads a cell it has passed.
+template <int STRIDE, int OSTRIDE, bool TO_GLOBAL, bool WANT_SPEED, bool ALIGNED = false>
 struct FinalSink {
     float* dst[NCOMP];       // TO_GLOBAL: &out[g][var(q)][..] at interior cell 0 of the row; else smem row (cell 0)
     float* fptr[NCOMP];
@@ -114,7 +117,18 @@ struct FinalSink {
     float held[NCOMP];
     template <int ODD>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
-        if (TO_GLOBAL) {
+        if ((TO_GLOBAL || ALIGNED) && STRIDE == 1) {
+            // backward pass, last sweep along x: a thread owns the 16 contiguous cells of its output row (64 B, aligned);
+            // interior cells i = j - 3 go out in pairs (i even, i + 1) as 64-bit stores: the odd padded cell waits
+            if (ODD) {
+#pragma unroll
+                for (int k = 0; k < NCOMP; ++k) held[k] = u[k];
+            } else {
+#pragma unroll
+                for (int k = 0; k < NCOMP; ++k)
+                    *reinterpret_cast<float2*>(dst[k] + (j - 1 - NG)) = make_float2(held[k], u[k]);
+            }
+        } else if (TO_GLOBAL) {
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) dst[k][(j - NG) * OSTRIDE] = u[k];
         } else if (STRIDE == 1 && !GAMER_X32) {
@@ -158,6 +172,10 @@ struct FinalSink {
         }
     }
 };
+
+// Offset (floats) from the start of a padded x row to the first 16-byte boundary of shared memory inside it: the row of
+// padded y starts 88 y bytes into its plane, so 0 for even y and 2 for odd y.
+__host__ __device__ constexpr int aligned_row_shift(int y) { return (y & 1) ? 2 : 0; }
 
 // Row-local component order (rho, m_n, m_t1, m_t2, e) -> variable index, for sweep axis d (0:x, 1:y, 2:z).
 __device__ __forceinline__ int var_of(int d, int q) {
@@ -211,12 +229,14 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
         sink.face_row = face_row;
         rtvd_march<STRIDE, WANT_FACE>(src, gc, sink, gate);
     } else {
-        FinalSink<STRIDE, OSTRIDE, LAST_TO_GLOBAL, WANT_SPEED> sink;
+        constexpr bool ALIGNED = D == 0 && !LAST_TO_GLOBAL;      // backward pass: x sweep in place, see FinalSink
+        FinalSink<STRIDE, OSTRIDE, LAST_TO_GLOBAL, WANT_SPEED, ALIGNED> sink;
 #pragma unroll
         for (int q = 0; q < NCOMP; ++q) {
+            // ALIGNED: cell j is written at j - 3 + aligned_row_shift(y); the sink indexes with j - 3
             sink.dst[q] = LAST_TO_GLOBAL
                               ? out_g + var_of(D, q) * (PS * PS * PS) + (a - NG) * OSTR_A + (b - NG) * OSTR_B
-                              : const_cast<float*>(src[q]);
+                              : const_cast<float*>(src[q]) + (ALIGNED ? aligned_row_shift(a) : 0);
             sink.fptr[q] = WANT_FACE ? face_g + ((D * 3) * NCOMP + var_of(D, q)) * (PS * PS) + (b - NG) * PS + (a - NG)
                                      : nullptr;
         }
@@ -308,6 +328,25 @@ __device__ __forceinline__ void load_chunk(float* smem, Ctl* ctl, const float* _
                  &ctl->full[c]);
 }
 
+// Backward pass (z,y,x): the z sweep comes first and needs the planes in order; after it the ghost planes 0-2 and 19-21
+// are dead (the y and x sweeps only touch z = 3..18), so the same planes of the CTA's NEXT group are loaded into them
+// under the y and x sweeps; the interior planes follow in four chunks once the x sweep has read them.
+constexpr int BCHUNK_PLANES = 4;                                  // interior planes per load chunk
+constexpr int N_BCHUNK = 2 + PS / BCHUNK_PLANES;                  // ghost planes below, interior chunks, ghost planes above
+__host__ __device__ constexpr int bchunk_lo(int c) { return c == 0 ? 0 : NG + BCHUNK_PLANES * (c - 1); }   // 0, 3, 7, 11, 15, 19
+__host__ __device__ constexpr int bchunk_hi(int c) {
+    return c == 0 ? NG : (c == N_BCHUNK - 1 ? NP : NG + BCHUNK_PLANES * c);
+}
+static_assert(bchunk_hi(N_BCHUNK - 2) == NG + PS && bchunk_lo(N_BCHUNK - 1) == NG + PS, "backward load chunks");
+// One thread calls this.
+__device__ __forceinline__ void load_bchunk(float* smem, Ctl* ctl, const float* __restrict__ in_g, int c) {
+    const int lo = bchunk_lo(c), bytes = (bchunk_hi(c) - lo) * PLANE_BYTES;
+    mbar_expect_tx(&ctl->full[c], NCOMP * bytes);
+#pragma unroll
+    for (int v = 0; v < NCOMP; ++v)
+        bulk_g2s(smem + v * VAR_FLOATS + lo * PLANE_FLOATS, in_g + v * VAR_FLOATS + lo * PLANE_FLOATS, bytes,
+                 &ctl->full[c]);
+}
 // Gate of the forward z march (the last sweep; its results go straight to HBM): once a thread has the last planes of
 // a load chunk in registers it never reads the chunk again and says so on BAR_ZFREE + c (bar.arrive: nothing in the
 // march waits).  The loader warp syncs on these barriers and starts the bulk copies of the same planes of the CTA's
@@ -322,12 +361,15 @@ struct ZPlaneGate {
     }
 };
 
-// Gate of the backward z march (the first sweep): wait for a load chunk when the march reaches its first plane.
+// Gate of the backward z march (the first sweep): wait for a load chunk when the march first reaches one of its planes.
+// The march reads planes n, n+1 (n even): chunk 0 at n = 0, chunk c >= 1 (first plane 4 c - 1) at n = 4 c - 2.
 struct ChunkWaitGate {
     Ctl* ctl;
     uint32_t parity;
     __device__ __forceinline__ void acquire(int n) {
-        if (n % (2 * CHUNK_PAIRS) == 0) mbar_wait_poll(&ctl->full[n / (2 * CHUNK_PAIRS)], parity);
+        static_assert(BCHUNK_PLANES == 4, "gate arithmetic");
+        if (n == 0) mbar_wait_poll(&ctl->full[0], parity);
+        else if ((n & 3) == 2) mbar_wait_poll(&ctl->full[(n + 2) >> 2], parity);
     }
     __device__ __forceinline__ void release(int) {}
 };
@@ -396,10 +438,12 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             ctl->zfin[i] = 0u;
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        if (!BACKWARD) {              // the first group of this CTA, plane by plane
-            fence_proxy_async();
-            const float* in_g = in + (long long)blockIdx.x * GROUP_IN_FLOATS;
+        fence_proxy_async();          // the first group of this CTA, chunk by chunk
+        const float* in_g = in + (long long)blockIdx.x * GROUP_IN_FLOATS;
+        if (!BACKWARD) {
             for (int c = 0; c < N_CHUNK; ++c) load_chunk(smem, ctl, in_g, c);
+        } else {
+            for (int c = 0; c < N_BCHUNK; ++c) load_bchunk(smem, ctl, in_g, c);
         }
     }
     __syncthreads();
@@ -439,35 +483,57 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             // no CTA-wide barrier: a plane is overwritten only after all z threads have read it (BAR_ZFREE), and the
             // next group's x tasks wait for their planes (BAR_FULL)
         } else {
-            // The group arrives in the same three chunks of z-planes; the z march (first sweep) waits for a chunk only
-            // when it reaches its first plane, so all but the first chunk land under the march.
-            if (threadIdx.x == 0) {
-                fence_proxy_async();  // generic-proxy accesses of the previous group are ordered before the async write
-                const float* in_g = in + g * (long long)GROUP_IN_FLOATS;
-                for (int c = 0; c < N_CHUNK; ++c) load_chunk(smem, ctl, in_g, c);
-                const long long gn = g + gridDim.x;
-                if (gn < n_groups) bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_BYTES);
-            }
+            // The group arrives in six chunks of z-planes (bchunk_lo/hi); the z march (first sweep) waits for a chunk
+            // only when it reaches its first plane.  All chunks of this group were issued earlier: by the prologue
+            // (first group of the CTA) or under / after the sweeps of the previous group.
+            // (Measured and rejected: the x march storing to HBM itself with 64-bit stores, 9 % slower — uncoalesced;
+            // a loader warp issuing the copies instead of thread 0, 2 % slower — every warp has z rows in the first
+            // sweep and a bulk copy holds its issuer for about as long as the transfer takes.)
+            const long long gn = g + gridDim.x;
+            const bool has_next = gn < n_groups;
+            const float* in_next = in + (has_next ? gn : g) * (long long)GROUP_IN_FLOATS;
+            if (threadIdx.x == 0 && has_next) bulk_prefetch_l2(in_next, GROUP_IN_BYTES);
             ChunkWaitGate zgate;
             zgate.ctl = ctl;
             zgate.parity = parity;
             sweep<2, 0, NP, 0, NP, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, zgate);
             __syncthreads();
+            // the ghost planes 0-2 and 19-21 are dead from here on: the next group's go in under the y and x sweeps
+            if (threadIdx.x == BLOCK_THREADS - 1 && has_next) {      // a thread without y or x rows
+                fence_proxy_async();
+                load_bchunk(smem, ctl, in_next, 0);
+                load_bchunk(smem, ctl, in_next, N_BCHUNK - 1);
+            }
             sweep<1, 0, NP, NG, PS, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
+            // last sweep: along x, in place; then a coalesced 128-bit copy-out of the interior, chunk by chunk, each
+            // chunk's planes handed to the bulk copies of the next group as soon as they have been read
             sweep<0, NG, PS, NG, PS, true, false, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
                                                                          nogate);
             if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);
             __syncthreads();
-            // coalesced 128-bit copy-out of the interior: 16 B = 4 cells of a 16-cell row (row start 3 is not 16-B
-            // aligned in shared memory, so read scalars, write float4)
-            for (int i = threadIdx.x; i < GROUP_OUT_FLOATS / 4; i += BLOCK_THREADS) {
-                const int x4 = i & 3, y = (i >> 2) & 15, z = (i >> 6) & 15, v = i >> 10;
-                const float* s = smem + v * VAR_FLOATS + (z + NG) * (NP * NP) + (y + NG) * NP + NG + 4 * x4;
-                float4 val = make_float4(s[0], s[1], s[2], s[3]);
-                reinterpret_cast<float4*>(out_g)[i] = val;
+            constexpr int PER_CHUNK = NCOMP * BCHUNK_PLANES * PS * 4;       // float4 per chunk
+#pragma unroll 1
+            for (int c = 1; c < N_BCHUNK - 1; ++c) {
+                // 16 B = 4 cells of a 16-cell row; the x sweep left each row on a 16-byte boundary (FinalSink ALIGNED)
+#pragma unroll
+                for (int i0 = 0; i0 < PER_CHUNK; i0 += BLOCK_THREADS) {
+                    const int i = i0 + threadIdx.x;
+                    if (i < PER_CHUNK) {
+                        const int x4 = i & 3, y = (i >> 2) & 15, zc = (i >> 6) % BCHUNK_PLANES, v = i / (64 * BCHUNK_PLANES);
+                        const int z = (c - 1) * BCHUNK_PLANES + zc;
+                        const float* sp = smem + v * VAR_FLOATS + (z + NG) * (NP * NP) + (y + NG) * NP +
+                                          aligned_row_shift(y + NG) + 4 * x4;
+                        reinterpret_cast<float4*>(out_g)[(v * PS + z) * (PS * 4) + y * 4 + x4] =
+                            *reinterpret_cast<const float4*>(sp);
+                    }
+                }
+                __syncthreads();          // every thread is done with the chunk before the bulk copy overwrites it
+                if (threadIdx.x == 0 && has_next) {
+                    fence_proxy_async();
+                    load_bchunk(smem, ctl, in_next, c);
+                }
             }
-            __syncthreads();          // every thread is done with the buffer before the next bulk copy overwrites it
         }
     }
 }
