@@ -324,8 +324,11 @@ int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int
     if (d_interior == nullptr || d_padded == nullptr) return fail(GAMER_EINVAL, "NULL pointer");
     if (!aligned16(d_interior) || !aligned16(d_padded)) return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
     g_err[0] = '\0';
+    int sm_count = 0;
+    rc = prepare(reinterpret_cast<const void*>(gamer::ghost_fill_kernel), 13, gamer::GF_SMEM_BYTES, &sm_count);
+    if (rc != GAMER_OK) return rc;
     gamer::BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
-    gamer::ghost_fill_kernel<<<(unsigned int)gamer::ghost_fill_ctas(gx, gy, gz), gamer::GF_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
+    gamer::ghost_fill_kernel<<<(unsigned int)gamer::ghost_fill_ctas(gx, gy, gz), gamer::GF_THREADS, gamer::GF_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(
         d_interior, d_padded, geo);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "ghost_fill launch: %s", cudaGetErrorString(e));
@@ -361,6 +364,7 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     int sm_count = 0;
     rc = prepare(reinterpret_cast<const void*>(fwd), order == 0 ? 8 : 11, SMEM_BYTES, &sm_count);
     if (rc == GAMER_OK && order == 1) rc = prepare(reinterpret_cast<const void*>(bwd), 12, SMEM_BYTES, &sm_count);
+    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(ghost_fill_kernel), 13, GF_SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
     const int grid = (int)(n < (long long)sm_count ? n : (long long)sm_count);
     const int red_grid = (int)(n < 4ll * sm_count ? n : 4ll * sm_count);
@@ -382,11 +386,11 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
         fwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr,
                                                          order == 0 ? d_speed : nullptr, d_work + 1);
         if (order == 1) {       // the backward sweep z,y,x follows with the SAME time step
-            ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
+            ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
             bwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr, d_speed, d_work + 1);
         }
         group_speed_max_kernel<<<gsm_grid, 256, 0, stream>>>(d_speed, n, acc);
-        ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, 0, stream>>>(d_interior, d_padded, geo);
+        ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "run_uniform: %s", cudaGetErrorString(e));

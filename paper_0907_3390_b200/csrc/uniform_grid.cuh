@@ -16,36 +16,34 @@ struct BoxGeom {
     int bc[3];               // per axis x, y, z: 0 = periodic, 1 = leave the ghost cells beyond the box untouched
 };
 
-// One CTA per (group, variable).  The 22^3 padded cells of that variable are assembled in shared memory — per (z,y)
-// row: the 16 interior cells as four 128-bit loads from the owning group's interior, 3 + 3 ghost cells from the x
-// neighbours; rows whose y or z lies beyond the box come from the y/z neighbours (periodic) or are re-read from the
-// padded array itself ("keep") — and then written out as one contiguous, 16-byte-aligned block with 128-bit stores.
+// One CTA per (strip of groups along x, variable): the CTA walks kx = 0 .. gx-1 and assembles the 22^3 padded cells of
+// one group and variable at a time in shared memory, then hands the contiguous, 16-byte-aligned 42 592-byte block to one
+// bulk store (TMA), so that the LSU pipe only sees the gather side.
+//   * Every global read is a 128-bit load of an aligned quarter of a 16-cell interior row (thread = (padded row, quarter);
+//     rows whose y or z lies beyond the box come from the y/z neighbours, periodic, or are re-read from the padded array
+//     itself, "keep").
+//   * The ghost cells x = 0..2 of group kx are cells 13..15 of the same rows of group kx-1 and x = 19..21 are cells 0..2
+//     of group kx+1: the threads that loaded those quarters one step earlier / later write them, so no separate load
+//     of the x neighbours exists (the first version spent a quarter of its time on those 12-byte reads).  The walk
+//     therefore runs from kx = -1 (wrap: only remembered) to kx = gx (wrap: only its first quarters are used), and two
+//     tiles are in flight: tile kx is being filled while tile kx-1 receives its last ghost cells and leaves.
 constexpr int GF_THREADS = 256;
-constexpr int GF_TILE = 4;
+constexpr int GF_ROWS = NP * NP;                                  // 484 padded (z,y) rows
+constexpr int GF_ITEMS = (GF_ROWS * 4 + GF_THREADS - 1) / GF_THREADS;   // 8 quarter rows per thread (the last one partial)
+constexpr int GF_SMEM_BYTES = 2 * VAR_FLOATS * 4 + 2 * NP * 8;    // two tiles + the y and z offset tables
 // number of CTAs that ghost_fill_kernel needs for a box of gx x gy x gz groups
-inline long long ghost_fill_ctas(int gx, int gy, int gz) {
-    auto up = [](int a) { return (long long)((a + GF_TILE - 1) / GF_TILE); };
-    return up(gx) * up(gy) * up(gz) * GF_TILE * GF_TILE * GF_TILE * NCOMP;
-}
-__global__ void __launch_bounds__(GF_THREADS)
+inline long long ghost_fill_ctas(int gx, int gy, int gz) { (void)gx; return (long long)gy * gz * NCOMP; }
+
+__global__ void __launch_bounds__(GF_THREADS, 2)
 ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded, BoxGeom geo) {
-    __shared__ __align__(16) float tile[VAR_FLOATS];
-    // CTAs walk the box in 4 x 4 x 4 tiles of groups, so that the neighbours whose interiors a group reads are
-    // handled close in time and the reads hit L2 (in plain group order the z neighbours are gx*gy groups apart)
+    extern __shared__ __align__(128) unsigned char gf_smem[];
+    float* const tiles = reinterpret_cast<float*>(gf_smem);                       // [2][VAR_FLOATS]
+    long long* const off_y = reinterpret_cast<long long*>(gf_smem + 2 * VAR_FLOATS * 4);
+    long long* const off_z = off_y + NP;
     const int v = blockIdx.x % NCOMP;
-    const long long q = blockIdx.x / NCOMP;
-    const int ntx = (geo.gx + GF_TILE - 1) / GF_TILE, nty = (geo.gy + GF_TILE - 1) / GF_TILE;
-    const long long tile_id = q / (GF_TILE * GF_TILE * GF_TILE);
-    const int w = (int)(q % (GF_TILE * GF_TILE * GF_TILE));
-    const int kx = (int)(tile_id % ntx) * GF_TILE + w % GF_TILE;
-    const int ky = (int)((tile_id / ntx) % nty) * GF_TILE + (w / GF_TILE) % GF_TILE;
-    const int kz = (int)(tile_id / ((long long)ntx * nty)) * GF_TILE + w / (GF_TILE * GF_TILE);
-    if (kx >= geo.gx || ky >= geo.gy || kz >= geo.gz) return;
-    const long long g = ((long long)kz * geo.gy + ky) * geo.gx + kx;
-    float* dst = padded + (g * NCOMP + v) * (long long)VAR_FLOATS;
-    // Per padded y and z: offset (in floats) of the source row inside `interior`, or -1 = beyond a "keep" end.  The
-    // index arithmetic is done once per CTA here, not once per cell (the first version was bound by it).
-    __shared__ long long off_y[NP], off_z[NP];
+    const int strip = blockIdx.x / NCOMP;
+    const int ky = strip % geo.gy, kz = strip / geo.gy;
+    // Per padded y and z: offset (in floats) of the source row inside `interior`, or -1 = beyond a "keep" end.
     constexpr long long GS = (long long)NCOMP * PS * PS * PS;     // floats per group of `interior`
     if (threadIdx.x < 2 * NP) {
         const bool is_z = threadIdx.x >= NP;
@@ -60,41 +58,87 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
         (is_z ? off_z : off_y)[p] = keep ? -1 : off;
     }
     __syncthreads();
-    // x: own group, left and right neighbour (or -1 = beyond a "keep" end)
-    const int kxl = kx > 0 ? kx - 1 : (geo.bc[0] ? -1 : geo.gx - 1);
-    const int kxr = kx < geo.gx - 1 ? kx + 1 : (geo.bc[0] ? -1 : 0);
-    const float* const src_c = interior + kx * GS + v * (PS * PS * PS);
-    const float* const src_l = kxl < 0 ? nullptr : interior + kxl * GS + v * (PS * PS * PS) + (PS - NG);
-    const float* const src_r = kxr < 0 ? nullptr : interior + kxr * GS + v * (PS * PS * PS) - (PS + NG);
-    // (1) the 16 cells x = 3..18 of every row: four 128-bit loads per row
-#pragma unroll 4
-    for (int t = threadIdx.x; t < NP * NP * 4; t += GF_THREADS) {
-        const int row = t >> 2, part = t & 3;
-        const int z = row / NP, y = row - z * NP;
-        const long long oy = off_y[y], oz = off_z[z];
-        float* trow = tile + row * NP + NG + 4 * part;
-        float4 q;
-        if (oy >= 0 && oz >= 0) {
-            q = *reinterpret_cast<const float4*>(src_c + oz + oy + 4 * part);
-        } else {
-            const float* d = dst + row * NP + NG + 4 * part;
-            q = make_float4(d[0], d[1], d[2], d[3]);
+    const int part = threadIdx.x & 3;                              // quarter of the 16-cell row, the same for all items
+    const float* const src_v = interior + v * (PS * PS * PS) + 4 * part;
+    long long row_off[GF_ITEMS];                                   // source offset of this thread's rows, -1 = keep
+#pragma unroll
+    for (int k = 0; k < GF_ITEMS; ++k) {
+        const int row = (threadIdx.x >> 2) + (GF_THREADS / 4) * k;
+        row_off[k] = -1;
+        if (row < GF_ROWS) {
+            const int z = row / NP, y = row - z * NP;
+            const long long oy = off_y[y], oz = off_z[z];
+            row_off[k] = (oy >= 0 && oz >= 0) ? oy + oz : -1;
         }
-        trow[0] = q.x; trow[1] = q.y; trow[2] = q.z; trow[3] = q.w;
     }
-    // (2) the ghost cells x = 0..2 (left neighbour's cells 13..15) and x = 19..21 (right neighbour's cells 0..2)
-#pragma unroll 2
-    for (int t = threadIdx.x; t < NP * NP * 2 * NG; t += GF_THREADS) {
-        const int row = t / (2 * NG), j = t - row * (2 * NG);
-        const int z = row / NP, y = row - z * NP;
-        const long long oy = off_y[y], oz = off_z[z];
-        const int x = j < NG ? j : PS + j;                        // padded x: 0..2 or 19..21
-        const float* sx = j < NG ? src_l : src_r;                 // sx[x] is the source cell of padded x
-        tile[row * NP + x] = (oy >= 0 && oz >= 0 && sx != nullptr) ? sx[oz + oy + x] : dst[row * NP + x];
+    const long long g0 = ((long long)kz * geo.gy + ky) * geo.gx;  // group index of kx = 0 in this strip
+    float4 prev[GF_ITEMS];                                         // the quarters loaded one step earlier (group kx-1)
+    for (int kx = -1; kx <= geo.gx; ++kx) {
+        const int ks = kx < 0 ? geo.gx - 1 : (kx == geo.gx ? 0 : kx);          // group whose interior is read (wrap)
+        const bool fill = kx >= 0 && kx < geo.gx;                                // tile kx exists
+        const bool wrap_l = kx == 0 && geo.bc[0], wrap_r = kx == geo.gx && geo.bc[0];   // "keep" ends along x
+        float* const tile = tiles + (kx & 1) * VAR_FLOATS;                      // tile of group kx
+        float* const tprev = tiles + ((kx + 1) & 1) * VAR_FLOATS;               // tile of group kx-1
+        float* const dst = padded + ((g0 + (fill ? kx : 0)) * NCOMP + v) * (long long)VAR_FLOATS;
+        float* const dprev = padded + ((g0 + (kx > 0 ? kx - 1 : 0)) * NCOMP + v) * (long long)VAR_FLOATS;
+        // the bulk store that last read `tile` (group kx-2) must have finished reading before anybody writes to it
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+        const float* const src = src_v + ks * GS;
+        float4 q[GF_ITEMS];
+        // only the quarters that are used are loaded: all of them for a tile, the first / last ones at the two wraps
+        const bool need = fill || (kx < 0 && part == 3) || (kx == geo.gx && part == 0);
+#pragma unroll
+        for (int k = 0; k < GF_ITEMS; ++k) {
+            const int row = (threadIdx.x >> 2) + (GF_THREADS / 4) * k;
+            q[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (row < GF_ROWS && need && row_off[k] >= 0) q[k] = __ldg(reinterpret_cast<const float4*>(src + row_off[k]));
+        }
+#pragma unroll
+        for (int k = 0; k < GF_ITEMS; ++k) {
+            const int row = (threadIdx.x >> 2) + (GF_THREADS / 4) * k;
+            if (row < GF_ROWS) {
+                const bool keep_row = row_off[k] < 0;              // y or z beyond a "keep" end: the whole row is kept
+                if (fill) {
+                    float* o = tile + row * NP + NG + 4 * part;
+                    if (keep_row) {
+                        const float* e = dst + row * NP + NG + 4 * part;
+                        q[k] = make_float4(e[0], e[1], e[2], e[3]);
+                    }
+                    o[0] = q[k].x; o[1] = q[k].y; o[2] = q[k].z; o[3] = q[k].w;
+                    if (part == 3) {                               // ghost cells x = 0..2: cells 13..15 of group kx-1
+                        float* l = tile + row * NP;
+                        if (keep_row || wrap_l) {
+                            const float* e = dst + row * NP;
+                            l[0] = e[0]; l[1] = e[1]; l[2] = e[2];
+                        } else {
+                            l[0] = prev[k].y; l[1] = prev[k].z; l[2] = prev[k].w;
+                        }
+                    }
+                }
+                if (kx > 0 && part == 0) {                         // ghost cells x = 19..21 of group kx-1: cells 0..2 here
+                    float* r = tprev + row * NP + NG + PS;
+                    if (keep_row || wrap_r) {
+                        const float* e = dprev + row * NP + NG + PS;
+                        r[0] = e[0]; r[1] = e[1]; r[2] = e[2];
+                    } else {
+                        r[0] = q[k].x; r[1] = q[k].y; r[2] = q[k].z;
+                    }
+                }
+            }
+            prev[k] = q[k];
+        }
+        // tile kx-1 is complete: make the generic-proxy writes visible to the async proxy and let it go
+        fence_proxy_async();
+        __syncthreads();
+        if (threadIdx.x == 0 && kx > 0) {
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dprev), "r"(smem_u32(tprev)),
+                         "r"(VAR_FLOATS * 4)
+                         : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
     }
-    __syncthreads();
-    for (int i = threadIdx.x; i < VAR_FLOATS / 4; i += GF_THREADS)
-        reinterpret_cast<float4*>(dst)[i] = reinterpret_cast<const float4*>(tile)[i];
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the tiles must outlive the reads
 }
 
 // max of c_s + max(|v_x|,|v_y|,|v_z|) (Eq.30) as the bit pattern of a non-negative float in *acc (atomicMax on
