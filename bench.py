@@ -98,16 +98,15 @@ class ClockSampler(threading.Thread):
                     samples=len(self.samples))
 
 
-def kernel_source_hash():
-    """sha256 (first 16 hex digits) over the CUDA sources of the library, in name order: identifies the kernel build
-    that a profiles/*_traffic.csv row was captured on."""
+def kernel_source_hash(files=("rtvd_march.cuh", "hydro_kernel.cuh")):
+    """sha256 (first 16 hex digits) over the CUDA sources of the fp32 hydro kernel (the row march and the kernel around
+    it): identifies the kernel build that a profiles/*_traffic.csv row was captured on."""
     import hashlib
     h = hashlib.sha256()
     cdir = os.path.join(ROOT, "paper_0907_3390_b200", "csrc")
-    for fn in sorted(os.listdir(cdir)):
-        if fn.endswith((".cu", ".cuh")):
-            h.update(fn.encode())
-            h.update(open(os.path.join(cdir, fn), "rb").read())
+    for fn in files:
+        h.update(fn.encode())
+        h.update(open(os.path.join(cdir, fn), "rb").read())
     return h.hexdigest()[:16]
 
 

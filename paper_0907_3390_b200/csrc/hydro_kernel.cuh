@@ -104,10 +104,7 @@ struct SmemSink {
 
 // Writes the updated cells of the LAST sweep.  TO_GLOBAL: straight to out[g][v][.][.][.] with element stride OSTRIDE
 // along the row; else in place in shared memory.  Tracks the CFL speed of the updated cells if WANT_SPEED.
-// ALIGNED (backward pass, x sweep in place): the 16 new cells of a row are written 3 (even y) or 1 (odd y) cells to the
-// left of where they belong, i.e. starting on a 16-byte boundary of shared memory, so that the copy-out reads them
-// with 128-bit loads; dst[] already carries that shift.  Safe in place: the march never re-reads a cell it has passed.
-template <int STRIDE, int OSTRIDE, bool TO_GLOBAL, bool WANT_SPEED, bool ALIGNED = false>
+template <int STRIDE, int OSTRIDE, bool TO_GLOBAL, bool WANT_SPEED>
 struct FinalSink {
     float* dst[NCOMP];       // TO_GLOBAL: &out[g][var(q)][..] at interior cell 0 of the row; else smem row (cell 0)
     float* fptr[NCOMP];
@@ -117,7 +114,7 @@ struct FinalSink {
     float held[NCOMP];
     template <int ODD>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
-        if ((TO_GLOBAL || ALIGNED) && STRIDE == 1) {
+        if (TO_GLOBAL && STRIDE == 1) {
             // backward pass, last sweep along x: a thread owns the 16 contiguous cells of its output row (64 B, aligned);
             // interior cells i = j - 3 go out in pairs (i even, i + 1) as 64-bit stores: the odd padded cell waits
             if (ODD) {
@@ -173,10 +170,6 @@ struct FinalSink {
     }
 };
 
-// Offset (floats) from the start of a padded x row to the first 16-byte boundary of shared memory inside it: the row of
-// padded y starts 88 y bytes into its plane, so 0 for even y and 2 for odd y.
-__host__ __device__ constexpr int aligned_row_shift(int y) { return (y & 1) ? 2 : 0; }
-
 // Row-local component order (rho, m_n, m_t1, m_t2, e) -> variable index, for sweep axis d (0:x, 1:y, 2:z).
 __device__ __forceinline__ int var_of(int d, int q) {
     return q == 0 ? 0 : (q == 4 ? 4 : 1 + (d + q - 1) % 3);
@@ -206,6 +199,17 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
         const int w = t >> 5, h = (t >> 4) & 1;
         a = LO_A + (t & 15);
         b = w < 10 ? 8 * (w >> 2) + (w & 3) + 4 * h : 18 + h;
+    } else if (D == 1 && N_A == NP && N_B == PS) {
+        // backward y sweep: 22 x columns x 16 planes.  x = 0..15 as above (the half-warps 4 planes = 16 banks apart);
+        // x = 16..21: six columns of planes that are two apart (a plane is 4 banks on, 6 columns fit in the 8)
+        if (t < PS * PS) {
+            a = t & 15;
+            b = LO_B + 8 * (t >> 7) + ((t >> 5) & 3) + 4 * ((t >> 4) & 1);
+        } else {
+            const int r = t - PS * PS, zi = r / 6;
+            a = PS + r - 6 * zi;
+            b = LO_B + 2 * (zi & 7) + (zi >> 3);
+        }
     } else if (D == 2 && N_A == PS && N_B == PS) {
         a = LO_A + (t & 15);
         b = LO_B + (t >> 5) + 8 * ((t >> 4) & 1);
@@ -229,14 +233,12 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
         sink.face_row = face_row;
         rtvd_march<STRIDE, WANT_FACE>(src, gc, sink, gate);
     } else {
-        constexpr bool ALIGNED = D == 0 && !LAST_TO_GLOBAL;      // backward pass: x sweep in place, see FinalSink
-        FinalSink<STRIDE, OSTRIDE, LAST_TO_GLOBAL, WANT_SPEED, ALIGNED> sink;
+        FinalSink<STRIDE, OSTRIDE, LAST_TO_GLOBAL, WANT_SPEED> sink;
 #pragma unroll
         for (int q = 0; q < NCOMP; ++q) {
-            // ALIGNED: cell j is written at j - 3 + aligned_row_shift(y); the sink indexes with j - 3
             sink.dst[q] = LAST_TO_GLOBAL
                               ? out_g + var_of(D, q) * (PS * PS * PS) + (a - NG) * OSTR_A + (b - NG) * OSTR_B
-                              : const_cast<float*>(src[q]) + (ALIGNED ? aligned_row_shift(a) : 0);
+                              : const_cast<float*>(src[q]);
             sink.fptr[q] = WANT_FACE ? face_g + ((D * 3) * NCOMP + var_of(D, q)) * (PS * PS) + (b - NG) * PS + (a - NG)
                                      : nullptr;
         }
@@ -515,17 +517,19 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             constexpr int PER_CHUNK = NCOMP * BCHUNK_PLANES * PS * 4;       // float4 per chunk
 #pragma unroll 1
             for (int c = 1; c < N_BCHUNK - 1; ++c) {
-                // 16 B = 4 cells of a 16-cell row; the x sweep left each row on a 16-byte boundary (FinalSink ALIGNED)
+                // 16 B = 4 cells of a 16-cell row; a row starts at cell 3, 4 bytes off an 8-byte boundary of shared memory:
+                // scalar, 64-bit, scalar (shifting the rows onto 16-byte boundaries costs the x march its
+                // conflict-free 64-bit stores: no gain)
 #pragma unroll
                 for (int i0 = 0; i0 < PER_CHUNK; i0 += BLOCK_THREADS) {
                     const int i = i0 + threadIdx.x;
                     if (i < PER_CHUNK) {
                         const int x4 = i & 3, y = (i >> 2) & 15, zc = (i >> 6) % BCHUNK_PLANES, v = i / (64 * BCHUNK_PLANES);
                         const int z = (c - 1) * BCHUNK_PLANES + zc;
-                        const float* sp = smem + v * VAR_FLOATS + (z + NG) * (NP * NP) + (y + NG) * NP +
-                                          aligned_row_shift(y + NG) + 4 * x4;
+                        const float* sp = smem + v * VAR_FLOATS + (z + NG) * (NP * NP) + (y + NG) * NP + NG + 4 * x4;
+                        const float2 mid = *reinterpret_cast<const float2*>(sp + 1);
                         reinterpret_cast<float4*>(out_g)[(v * PS + z) * (PS * 4) + y * 4 + x4] =
-                            *reinterpret_cast<const float4*>(sp);
+                            make_float4(sp[0], mid.x, mid.y, sp[3]);
                     }
                 }
                 __syncthreads();          // every thread is done with the chunk before the bulk copy overwrites it
