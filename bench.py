@@ -382,10 +382,13 @@ def run_ours(args):
         if rep > 1 and n4 * rep * (BYTES_PER_GROUP) < 12e9:
             d4r = d4.repeat(rep, 1, 1, 1, 1)
             o4r = torch.empty((n4 * rep, 5, 16, 16, 16), dtype=torch.float32, device=device)
-            ms4r = time_advance(hydro, torch, stream, d4r, o4r, n4 * rep, c4["dt"], c4["dh"], c4["gamma"], steps=10)
+            sampler4 = ClockSampler(physical_gpu_index(local), period=0.005)
+            sampler4.start()
+            ms4r = time_advance(hydro, torch, stream, d4r, o4r, n4 * rep, c4["dt"], c4["dh"], c4["gamma"], steps=40)
+            clocks4 = sampler4.stop()
             config4["tiled_x%d" % rep] = dict(n_groups=n4 * rep, ns_per_group=ms4r * 1e6 / (n4 * rep),
                                               frac=(n4 * rep * FLOPS_PER_GROUP / (ms4r * 1e-3) / 1e12) / fp32_peak_tflops,
-                                              ratio_to_config5=(ms4r / (n4 * rep)) / (kernel_ms / n))
+                                              ratio_to_config5=(ms4r / (n4 * rep)) / (kernel_ms / n), clocks=clocks4)
             del d4r, o4r
         del d4, o4, c4
         torch.cuda.empty_cache()
