@@ -4,15 +4,23 @@
 // Same row march as the fp32 kernel (rtvd_march.cuh, T = double).  A padded group in fp64 is 425 920 B and does not fit
 // in shared memory, so the pass is cut where the method allows it: the x and y sweeps act inside one z-plane
 // (PAPER.md:174-178), so they run on two halves of 11 planes (212 960 B each, bulk-copied by TMA); what the z sweep
-// needs of their result — the 16 x 16 interior columns of all 22 planes, 225 280 B — goes through a per-CTA scratch
-// block in device memory (L2-resident: 33 MB for 148 CTAs) and comes back as one shared-memory block for the z sweep,
-// which writes the interior straight to HBM.  One persistent CTA per SM, 256 threads (up to 255 registers: the
-// march state is twice as wide in fp64).  Traffic per group: 425 920 B in + 163 840 B out (+ 2 x 225 280 B of scratch
-// that stays in L2).
+// needs of their result — the 16 x 16 interior columns of all 22 planes, 225 280 B — is parked in TENSOR MEMORY: a z
+// row (22 cells x 5 variables x 2 words = 220 words) belongs to one thread from the moment the y sweep has produced it,
+// and tcgen05.ld/st move 32-bit words between a thread's registers and "its" TMEM lane (512 columns per lane, two z
+// warps per lane quadrant: 2 x 220 columns).  After the y sweep of a half every z thread copies its 11 planes' cells
+// from shared memory into its lane; the z march then reads its row from there and writes the interior straight to HBM.
+// Shared memory is free during the z sweep, so the first half of the CTA's next group is loaded under it.  One
+// persistent CTA per SM, 256 threads (up to 255 registers: the march state is twice as wide in fp64).  Traffic per
+// group: 425 920 B in + 163 840 B out.  (Round 1 passed the z block through a scratch block in device memory and read
+// it back: 403 ns/group.)
 #pragma once
 #include <cstdint>
 
 #include "hydro_kernel.cuh"
+
+#ifndef GAMER_F64_PREFETCH
+#define GAMER_F64_PREFETCH 1
+#endif
 
 namespace gamer {
 
@@ -28,6 +36,63 @@ constexpr int FWD_SCRATCH_DOUBLES = NCOMP * ZBUF_VAR;                // 28 160 p
 constexpr int F64_SCRATCH_DOUBLES = BWD_SCRATCH_DOUBLES;             // what the caller provides per CTA
 constexpr int F64_DATA_BYTES = FWD_SCRATCH_DOUBLES * 8;              // 225 280 (>= 5 * 5324 * 8 = 212 960)
 constexpr int F64_SMEM_BYTES = F64_DATA_BYTES + 64;
+
+
+// ---- tensor memory (tcgen05) as per-thread row storage ----------------------------------------------------------
+// 32x32b shape: thread i of a warp accesses lane (32 * (warp % 4) + i), N consecutive 32-bit columns from the address.
+__device__ __forceinline__ void tmem_alloc_all(uint32_t* smem_slot) {        // one warp; writes the base address
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_slot)), "r"(512u)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_all(uint32_t taddr) {           // the same warp
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(512u) : "memory");
+}
+__device__ __forceinline__ void tmem_st2(uint32_t taddr, const uint32_t (&r)[2]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]),
+                 "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+constexpr int ZROW_WORDS_PER_PLANE = 2 * NCOMP;                      // 10 columns: one cell, five doubles
+constexpr int ZROW_COLS = NP * ZROW_WORDS_PER_PLANE;                 // 220 columns per z row
+constexpr int ZROW_COL_STRIDE = 256;                                 // second z warp of a lane quadrant
+
+// Row source of the z march: this thread's row in tensor memory, [plane][row-local component][lo, hi].
+struct TmemRowSrc {
+    uint32_t taddr;                                                  // lane quadrant and first column of the row
+    __device__ __forceinline__ void load(int n, double (&ua)[NCOMP], double (&ub)[NCOMP]) const {
+        uint32_t a[16], b[4];
+        tmem_ld16(taddr + n * ZROW_WORDS_PER_PLANE, a);
+        tmem_ld4(taddr + n * ZROW_WORDS_PER_PLANE + 16, b);
+        tmem_wait_ld();
+#pragma unroll
+        for (int k = 0; k < NCOMP; ++k) ua[k] = __hiloint2double((int)a[2 * k + 1], (int)a[2 * k]);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) ub[k] = __hiloint2double((int)a[10 + 2 * k + 1], (int)a[10 + 2 * k]);
+        ub[3] = __hiloint2double((int)b[1], (int)b[0]);
+        ub[4] = __hiloint2double((int)b[3], (int)b[2]);
+    }
+};
 
 template <int STRIDE>
 struct SrcF64 {
@@ -70,28 +135,38 @@ __device__ __forceinline__ void march_f64(double* const (&row)[NCOMP], double* c
 
 __global__ void __launch_bounds__(F64_THREADS, 1)
 hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out, long long n_groups,
-                         GasConstT<double> gc, double* __restrict__ scratch) {
+                         GasConstT<double> gc, double* __restrict__ /*scratch: the backward pass uses it*/) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* buf = reinterpret_cast<double*>(smem_raw);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + F64_DATA_BYTES);
-    double* zblock = scratch + (long long)blockIdx.x * F64_SCRATCH_DOUBLES;
-    const int t = threadIdx.x;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + F64_DATA_BYTES + 16);
+    const int t = threadIdx.x, warp = t >> 5;
+    if (warp == 0) tmem_alloc_all(tmem_slot);
     if (t == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // first half of the first group
+        fence_proxy_async();
+        const double* in_g = in + (long long)blockIdx.x * GROUP_IN_FLOATS;
+        mbar_expect_tx(bar, NCOMP * HALF_VAR * 8);
+        for (int v = 0; v < NCOMP; ++v) bulk_g2s(buf + v * HALF_VAR, in_g + v * VAR_FLOATS, HALF_VAR * 8, bar);
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+    // this thread's z row (x = t & 15, y = t >> 4): lane quadrant warp % 4, lane = lane id, columns by warp / 4
+    const uint32_t zrow = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * ZROW_COL_STRIDE);
     uint32_t parity = 0;
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
         const double* in_g = in + g * (long long)GROUP_IN_FLOATS;
+        const long long gn = g + gridDim.x;
         for (int h = 0; h < 2; ++h) {
-            // ---- planes 11h .. 11h+10 of all variables into shared memory --------------------------------------
-            if (t == 0) {
-                fence_proxy_async();
-                mbar_expect_tx(bar, NCOMP * HALF_VAR * 8);
-                for (int v = 0; v < NCOMP; ++v)
-                    bulk_g2s(buf + v * HALF_VAR, in_g + v * VAR_FLOATS + h * HALF_VAR, HALF_VAR * 8, bar);
-            }
+            // ---- planes 11h .. 11h+10 of all variables are on their way into shared memory (issued earlier) -------
+#if GAMER_F64_PREFETCH
+            if (t == F64_THREADS - 1 && h == 0)          // the other half into L2 meanwhile (a thread without x rows)
+                for (int v = 0; v < NCOMP; ++v) bulk_prefetch_l2(in_g + v * VAR_FLOATS + HALF_VAR, HALF_VAR * 8);
+#endif
             mbar_wait_poll(bar, parity);
             parity ^= 1u;
             // ---- x sweep: 11 x 22 rows (y,z), in place --------------------------------------------------------
@@ -111,32 +186,61 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
                 march_f64<NP, 0>(row, row, gc);
             }
             __syncthreads();
-            // ---- the 16 x 16 interior columns of these planes -> scratch block [v][z][j][i] ---------------------
-            for (int i = t; i < NCOMP * HALF_PLANES * PS * PS; i += F64_THREADS) {
-                const int x = i & 15, y = (i >> 4) & 15, zv = i >> 8, z = zv % HALF_PLANES, v = zv / HALF_PLANES;
-                zblock[v * ZBUF_VAR + (h * HALF_PLANES + z) * (PS * PS) + y * PS + x] =
-                    buf[v * HALF_VAR + z * (NP * NP) + (y + NG) * NP + x + NG];
+            // ---- every z thread parks the cells of its column in these planes in tensor memory -------------------
+            {
+                const int x = t & 15, y = t >> 4;
+                const double* col = buf + (y + NG) * NP + x + NG;
+#pragma unroll 1
+                for (int z = 0; z < HALF_PLANES; ++z) {
+                    uint32_t w8[8], w2[2];
+#pragma unroll
+                    for (int q = 0; q < NCOMP; ++q) {
+                        const double val = col[var_of(2, q) * HALF_VAR + z * (NP * NP)];
+                        if (q < 4) {
+                            w8[2 * q] = (uint32_t)__double2loint(val);
+                            w8[2 * q + 1] = (uint32_t)__double2hiint(val);
+                        } else {
+                            w2[0] = (uint32_t)__double2loint(val);
+                            w2[1] = (uint32_t)__double2hiint(val);
+                        }
+                    }
+                    const uint32_t at = zrow + (uint32_t)((h * HALF_PLANES + z) * ZROW_WORDS_PER_PLANE);
+                    tmem_st8(at, w8);
+                    tmem_st2(at + 8, w2);
+                }
+                tmem_wait_st();
             }
-            __syncthreads();
+            __syncthreads();          // shared memory is free: the other half (or the next group's first half) may land
+            if (t == 0) {
+                const double* src = h == 0 ? in_g + HALF_VAR : (gn < n_groups ? in + gn * (long long)GROUP_IN_FLOATS : nullptr);
+                if (src != nullptr) {
+                    fence_proxy_async();
+                    mbar_expect_tx(bar, NCOMP * HALF_VAR * 8);
+                    for (int v = 0; v < NCOMP; ++v) bulk_g2s(buf + v * HALF_VAR, src + v * VAR_FLOATS, HALF_VAR * 8, bar);
+                }
+            }
         }
-        // ---- z sweep on the block (read back through the generic proxy: written by this CTA before the barrier) ----
-        for (int i = t; i < FWD_SCRATCH_DOUBLES / 2; i += F64_THREADS)
-            reinterpret_cast<double2*>(buf)[i] = reinterpret_cast<const double2*>(zblock)[i];
-        __syncthreads();
+        // ---- z sweep from tensor memory, results straight to HBM (the next group's first half lands meanwhile) -----
         {
             const int x = t & 15, y = t >> 4;
-            double* row[NCOMP];
             double* dst[NCOMP];
             double* out_g = out + g * (long long)GROUP_OUT_FLOATS;
 #pragma unroll
-            for (int q = 0; q < NCOMP; ++q) {
-                row[q] = buf + var_of(2, q) * ZBUF_VAR + y * PS + x;
-                dst[q] = out_g + var_of(2, q) * (PS * PS * PS) + y * PS + x;
-            }
-            march_f64<PS * PS, NG>(row, dst, gc);
+            for (int q = 0; q < NCOMP; ++q) dst[q] = out_g + var_of(2, q) * (PS * PS * PS) + y * PS + x;
+            TmemRowSrc src;
+            src.taddr = zrow;
+            SinkF64<PS * PS, NG> sink;
+#pragma unroll
+            for (int q = 0; q < NCOMP; ++q) sink.dst[q] = dst[q];
+            NoGate gate;
+            RowMarch<false, decltype(sink), double> m;
+            m.run(src, gc, sink, gate);
         }
-        __syncthreads();
+        // no barrier: the next copy into tensor memory is by the same thread, after its own march
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) tmem_dealloc_all(tmem_base);
 }
 
 // Backward (z,y,x) order.  The z sweep comes first and couples all planes, but its rows are independent: it runs on
