@@ -243,75 +243,121 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
     if (warp == 0) tmem_dealloc_all(tmem_base);
 }
 
-// Backward (z,y,x) order.  The z sweep comes first and couples all planes, but its rows are independent: it runs on
-// two halves of 11 y rows (all x, all 22 planes: 212 960 B each); the 16 z-swept interior planes pass through the
-// scratch block; the y and x sweeps act inside a plane and run on two chunks of 8 planes (154 880 B), the x sweep
-// writing the interior to HBM.
-__global__ void __launch_bounds__(F64_THREADS, 1)
-hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restrict__ out, long long n_groups,
-                                  GasConstT<double> gc, double* __restrict__ scratch) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* buf = reinterpret_cast<double*>(smem_raw);
-    double* zplanes = scratch + (long long)blockIdx.x * F64_SCRATCH_DOUBLES;     // [v][k = 0..15][y][x]
-    const int t = threadIdx.x;
-    constexpr int HROWS = HALF_PLANES * NP;          // 242 (y,x) positions of a half
-    for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
-        const double* in_g = in + g * (long long)GROUP_IN_FLOATS;
-        for (int h = 0; h < 2; ++h) {
-            // ---- rows y = 11h .. 11h+10 of every plane: buf[v][z][yy][x] ---------------------------------------
-            for (int i = t; i < NCOMP * NP * HROWS; i += F64_THREADS) {
-                const int r = i % HROWS, vz = i / HROWS;                          // vz = v * 22 + z
-                buf[i] = in_g[vz * (NP * NP) + h * HROWS + r];
-            }
-            __syncthreads();
-            // ---- z sweep: 242 rows (y,x), stride 242, in place -------------------------------------------------
-            if (t < HROWS) {
-                double* row[NCOMP];
+// Backward (z,y,x) order, the mirror image of the forward kernel with x and z exchanged.  The z and y sweeps do not
+// couple different x, so they run on two SLABS of 11 x columns: the z march of a slab reads its rows straight from
+// device memory (a warp reads runs of 11 consecutive doubles of a plane: the rows are independent and every plane is
+// read exactly when the march gets there) and writes the 16 interior planes into shared memory, [v][k][y][xs]
+// (154 880 B); the y sweep works there in place; then every x-row owner (y, k) parks the slab's 11 cells of its row in
+// tensor memory (220 columns per row as in the forward kernel).  After both slabs the x march runs from tensor
+// memory and writes the interior to HBM.  Thread 255, which has no row in the z sweep, prefetches the CTA's next group
+// into L2.  (Before: strided loads of two y halves, a round trip of the z-swept planes through a scratch block in
+// device memory, y and x sweeps on two chunks of 8 planes: 765 ns/group.)
+constexpr int SLAB_X = NP / 2;                                       // 11 x columns per slab
+constexpr int SLAB_PLANE = NP * SLAB_X;                              // 242 doubles: one z-swept plane of a slab
+constexpr int SLAB_VAR = PS * SLAB_PLANE;                            // 3872 doubles: one variable of a slab
+static_assert(NCOMP * SLAB_VAR * 8 <= F64_DATA_BYTES, "slab fits");
+
+// Row source of the backward z march: this thread's column in device memory, plane stride NP * NP.
+struct GlobalColSrc {
+    const double* src[NCOMP];
+    __device__ __forceinline__ void load(int n, double (&ua)[NCOMP], double (&ub)[NCOMP]) const {
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) row[q] = buf + var_of(2, q) * (NP * HROWS) + t;
-                march_f64<HROWS, 0>(row, row, gc);
-            }
-            __syncthreads();
-            // ---- the 16 interior planes of this half -> scratch -------------------------------------------------
-            for (int i = t; i < NCOMP * PS * HROWS; i += F64_THREADS) {
-                const int r = i % HROWS, vk = i / HROWS, k = vk % PS, v = vk / PS;
-                zplanes[v * BWD_VAR + k * (NP * NP) + h * HROWS + r] = buf[(v * NP + k + NG) * HROWS + r];
-            }
-            __syncthreads();
-        }
-        for (int c = 0; c < PS / BWD_CHUNK_PLANES; ++c) {
-            // ---- planes k = 8c .. 8c+7 back from scratch: buf[v][kk][y][x] --------------------------------------
-            for (int i = t; i < NCOMP * BWD_CHUNK_VAR / 2; i += F64_THREADS) {
-                const int v = i / (BWD_CHUNK_VAR / 2), r = i % (BWD_CHUNK_VAR / 2);
-                reinterpret_cast<double2*>(buf)[i] =
-                    reinterpret_cast<const double2*>(zplanes + v * BWD_VAR + c * BWD_CHUNK_VAR)[r];
-            }
-            __syncthreads();
-            // ---- y sweep: all 22 x, 8 planes, in place ----------------------------------------------------------
-            if (t < BWD_CHUNK_PLANES * NP) {
-                const int x = t % NP, kk = t / NP;
-                double* row[NCOMP];
-#pragma unroll
-                for (int q = 0; q < NCOMP; ++q) row[q] = buf + var_of(1, q) * BWD_CHUNK_VAR + kk * (NP * NP) + x;
-                march_f64<NP, 0>(row, row, gc);
-            }
-            __syncthreads();
-            // ---- x sweep: y = 3..18, 8 planes, results straight to HBM ------------------------------------------
-            if (t < BWD_CHUNK_PLANES * PS) {
-                const int y = NG + (t & 15), kk = t >> 4;
-                double* row[NCOMP];
-                double* dst[NCOMP];
-                double* out_g = out + g * (long long)GROUP_OUT_FLOATS;
-#pragma unroll
-                for (int q = 0; q < NCOMP; ++q) {
-                    row[q] = buf + var_of(0, q) * BWD_CHUNK_VAR + kk * (NP * NP) + y * NP;
-                    dst[q] = out_g + var_of(0, q) * (PS * PS * PS) + (c * BWD_CHUNK_PLANES + kk) * (PS * PS) + (y - NG) * PS;
-                }
-                march_f64<1, NG>(row, dst, gc);
-            }
-            __syncthreads();
+        for (int k = 0; k < NCOMP; ++k) {
+            ua[k] = __ldg(src[k] + n * (NP * NP));
+            ub[k] = __ldg(src[k] + (n + 1) * (NP * NP));
         }
     }
+};
+
+__global__ void __launch_bounds__(F64_THREADS, 1)
+hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restrict__ out, long long n_groups,
+                                  GasConstT<double> gc, double* __restrict__ /*scratch: unused since round 2*/) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* buf = reinterpret_cast<double*>(smem_raw);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + F64_DATA_BYTES + 16);
+    const int t = threadIdx.x, warp = t >> 5;
+    if (warp == 0) tmem_alloc_all(tmem_slot);
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+    // this thread's x row (y = 3 + (t & 15), plane k = t >> 4): lane quadrant warp % 4, columns by warp / 4
+    const uint32_t xrow = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * ZROW_COL_STRIDE);
+    for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
+        const double* in_g = in + g * (long long)GROUP_IN_FLOATS;
+        const long long gn = g + gridDim.x;
+        for (int s = 0; s < 2; ++s) {
+            // ---- z sweep of the slab: 22 x 11 rows (y, xs), device memory -> shared memory (interior planes) ---------
+            if (t < NP * SLAB_X) {
+                const int y = t / SLAB_X, xs = t - y * SLAB_X;
+                GlobalColSrc src;
+                SinkF64<SLAB_PLANE, NG> sink;
+#pragma unroll
+                for (int q = 0; q < NCOMP; ++q) {
+                    src.src[q] = in_g + var_of(2, q) * VAR_FLOATS + y * NP + s * SLAB_X + xs;
+                    sink.dst[q] = buf + var_of(2, q) * SLAB_VAR + t;
+                }
+                NoGate gate;
+                RowMarch<false, decltype(sink), double> m;
+                m.run(src, gc, sink, gate);
+            } else if (t == F64_THREADS - 1 && s == 1 && gn < n_groups) {
+                bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_FLOATS * 8);
+            }
+            __syncthreads();
+            // ---- y sweep: 11 x columns x 16 planes, in place -------------------------------------------------------
+            if (t < SLAB_X * PS) {
+                const int k = t / SLAB_X, xs = t - k * SLAB_X;
+                double* row[NCOMP];
+#pragma unroll
+                for (int q = 0; q < NCOMP; ++q) row[q] = buf + var_of(1, q) * SLAB_VAR + k * SLAB_PLANE + xs;
+                march_f64<SLAB_X, 0>(row, row, gc);
+            }
+            __syncthreads();
+            // ---- every x-row owner parks the slab's cells of its row in tensor memory ----------------------------------
+            {
+                const int yi = t & 15, k = t >> 4;
+                const double* rowp = buf + k * SLAB_PLANE + (yi + NG) * SLAB_X;
+#pragma unroll 1
+                for (int xs = 0; xs < SLAB_X; ++xs) {
+                    uint32_t w8[8], w2[2];
+#pragma unroll
+                    for (int q = 0; q < NCOMP; ++q) {
+                        const double val = rowp[var_of(0, q) * SLAB_VAR + xs];
+                        if (q < 4) {
+                            w8[2 * q] = (uint32_t)__double2loint(val);
+                            w8[2 * q + 1] = (uint32_t)__double2hiint(val);
+                        } else {
+                            w2[0] = (uint32_t)__double2loint(val);
+                            w2[1] = (uint32_t)__double2hiint(val);
+                        }
+                    }
+                    const uint32_t at = xrow + (uint32_t)((s * SLAB_X + xs) * ZROW_WORDS_PER_PLANE);
+                    tmem_st8(at, w8);
+                    tmem_st2(at + 8, w2);
+                }
+                tmem_wait_st();
+            }
+            __syncthreads();          // the slab buffer is free again
+        }
+        // ---- x sweep from tensor memory, results straight to HBM ----------------------------------------------------
+        {
+            const int yi = t & 15, k = t >> 4;
+            double* out_g = out + g * (long long)GROUP_OUT_FLOATS;
+            TmemRowSrc src;
+            src.taddr = xrow;
+            SinkF64<1, NG> sink;
+#pragma unroll
+            for (int q = 0; q < NCOMP; ++q) sink.dst[q] = out_g + var_of(0, q) * (PS * PS * PS) + k * (PS * PS) + yi * PS;
+            NoGate gate;
+            RowMarch<false, decltype(sink), double> m;
+            m.run(src, gc, sink, gate);
+        }
+        // no barrier: the next copy into tensor memory is by the same thread, after its own march; the next z sweep
+        // writes shared memory, which nobody reads during the x sweep
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) tmem_dealloc_all(tmem_base);
 }
 
 }  // namespace gamer
