@@ -255,16 +255,43 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
 constexpr int SLAB_X = NP / 2;                                       // 11 x columns per slab
 constexpr int SLAB_PLANE = NP * SLAB_X;                              // 242 doubles: one z-swept plane of a slab
 constexpr int SLAB_VAR = PS * SLAB_PLANE;                            // 3872 doubles: one variable of a slab
-static_assert(NCOMP * SLAB_VAR * 8 <= F64_DATA_BYTES, "slab fits");
 
-// Row source of the backward z march: this thread's column in device memory, plane stride NP * NP.
-struct GlobalColSrc {
+// Row source of the backward z march: this thread's column in device memory, plane stride NP * NP, fetched two pairs
+// of cells ahead by cp.async (LDGSTS) into a private ring in shared memory — three slots of 2 cells x 5 variables per
+// thread, 61 440 B behind the slab — so that the march never waits for device memory and needs no registers for it.
+constexpr int XSTAGE_PITCH = PS + 1;                                 // 17
+static_assert(NCOMP * PS * PS * XSTAGE_PITCH * 8 <= F64_DATA_BYTES, "x-sweep staging fits");
+constexpr int RING_SLOTS = 3;
+constexpr int RING_DOUBLES = RING_SLOTS * 2 * NCOMP * F64_THREADS;   // 7680
+static_assert((NCOMP * SLAB_VAR + RING_DOUBLES) * 8 <= F64_DATA_BYTES, "slab + ring fit");
+struct RingColSrc {
     const double* src[NCOMP];
+    double* ring;                                                    // &ring[0][0][0][t]
+    __device__ __forceinline__ void fetch(int n) const {             // cells n, n+1 -> slot (n / 2) % 3
+        double* slot = ring + ((n >> 1) % RING_SLOTS) * (2 * NCOMP * F64_THREADS);
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(slot + (c * NCOMP + k) * F64_THREADS)),
+                             "l"(src[k] + (n + c) * (NP * NP))
+                             : "memory");
+    }
     __device__ __forceinline__ void load(int n, double (&ua)[NCOMP], double (&ub)[NCOMP]) const {
+        if (n == 0) {
+            fetch(0);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            fetch(2);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
+        if (n + 4 < NP) fetch(n + 4);
+        asm volatile("cp.async.commit_group;" ::: "memory");         // possibly empty: keeps the group count uniform
+        asm volatile("cp.async.wait_group 2;" ::: "memory");         // all but the two youngest groups: cells n, n+1 are here
+        const double* slot = ring + ((n >> 1) % RING_SLOTS) * (2 * NCOMP * F64_THREADS);
 #pragma unroll
         for (int k = 0; k < NCOMP; ++k) {
-            ua[k] = __ldg(src[k] + n * (NP * NP));
-            ub[k] = __ldg(src[k] + (n + 1) * (NP * NP));
+            ua[k] = slot[k * F64_THREADS];
+            ub[k] = slot[(NCOMP + k) * F64_THREADS];
         }
     }
 };
@@ -290,7 +317,8 @@ hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restr
             // ---- z sweep of the slab: 22 x 11 rows (y, xs), device memory -> shared memory (interior planes) ---------
             if (t < NP * SLAB_X) {
                 const int y = t / SLAB_X, xs = t - y * SLAB_X;
-                GlobalColSrc src;
+                RingColSrc src;
+                src.ring = buf + NCOMP * SLAB_VAR + t;
                 SinkF64<SLAB_PLANE, NG> sink;
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) {
@@ -339,21 +367,31 @@ hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restr
             }
             __syncthreads();          // the slab buffer is free again
         }
-        // ---- x sweep from tensor memory, results straight to HBM ----------------------------------------------------
+        // ---- x sweep from tensor memory.  A thread owns a whole output row, so stores straight from the march would
+        // put the lanes of a warp 128 B apart (32 sectors per store: 20 k cycles of the SM's store path per group).  The
+        // march writes into shared memory instead, transposed and padded — [v][k][i][y], pitch 17: conflict-free for the
+        // writers (lanes = y) and for the readers (lanes = i) — and a coalesced copy-out follows.
         {
             const int yi = t & 15, k = t >> 4;
-            double* out_g = out + g * (long long)GROUP_OUT_FLOATS;
             TmemRowSrc src;
             src.taddr = xrow;
-            SinkF64<1, NG> sink;
+            SinkF64<XSTAGE_PITCH, NG> sink;
 #pragma unroll
-            for (int q = 0; q < NCOMP; ++q) sink.dst[q] = out_g + var_of(0, q) * (PS * PS * PS) + k * (PS * PS) + yi * PS;
+            for (int q = 0; q < NCOMP; ++q) sink.dst[q] = buf + ((var_of(0, q) * PS + k) * PS) * XSTAGE_PITCH + yi;
             NoGate gate;
             RowMarch<false, decltype(sink), double> m;
             m.run(src, gc, sink, gate);
         }
-        // no barrier: the next copy into tensor memory is by the same thread, after its own march; the next z sweep
-        // writes shared memory, which nobody reads during the x sweep
+        __syncthreads();
+        {
+            double* out_g = out + g * (long long)GROUP_OUT_FLOATS;
+#pragma unroll 8
+            for (int idx = t; idx < GROUP_OUT_FLOATS; idx += F64_THREADS) {
+                const int i = idx & 15, yi = (idx >> 4) & 15, vk = idx >> 8;
+                out_g[idx] = buf[(vk * PS + i) * XSTAGE_PITCH + yi];
+            }
+        }
+        __syncthreads();          // the next z sweep writes the same shared memory
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
