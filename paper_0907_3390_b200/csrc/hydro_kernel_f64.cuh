@@ -56,6 +56,32 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8])
                  "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
                  : "memory");
 }
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]),
+                 "r"(r[3])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+                 : "memory");
+}
+// One slab of a row, 11 cells x 5 variables x 2 words = 110 consecutive columns, in six instructions: a tcgen05.st costs
+// the same few dozen cycles of the SM's tensor-memory port whatever its width (22 narrow stores per row took 13 % of
+// the kernel).
+__device__ __forceinline__ void tmem_st110(uint32_t taddr, const uint32_t (&w)[110]) {
+    tmem_st32(taddr, w);
+    tmem_st32(taddr + 32, w + 32);
+    tmem_st32(taddr + 64, w + 64);
+    {
+        const uint32_t t8[8] = {w[96], w[97], w[98], w[99], w[100], w[101], w[102], w[103]};
+        tmem_st8(taddr + 96, t8);
+    }
+    tmem_st4(taddr + 104, w + 104);
+    {
+        const uint32_t t2[2] = {w[108], w[109]};
+        tmem_st2(taddr + 108, t2);
+    }
+}
 __device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4]) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
@@ -190,24 +216,16 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
             {
                 const int x = t & 15, y = t >> 4;
                 const double* col = buf + (y + NG) * NP + x + NG;
-#pragma unroll 1
-                for (int z = 0; z < HALF_PLANES; ++z) {
-                    uint32_t w8[8], w2[2];
+                uint32_t w[HALF_PLANES * ZROW_WORDS_PER_PLANE];
+#pragma unroll
+                for (int z = 0; z < HALF_PLANES; ++z)
 #pragma unroll
                     for (int q = 0; q < NCOMP; ++q) {
                         const double val = col[var_of(2, q) * HALF_VAR + z * (NP * NP)];
-                        if (q < 4) {
-                            w8[2 * q] = (uint32_t)__double2loint(val);
-                            w8[2 * q + 1] = (uint32_t)__double2hiint(val);
-                        } else {
-                            w2[0] = (uint32_t)__double2loint(val);
-                            w2[1] = (uint32_t)__double2hiint(val);
-                        }
+                        w[z * ZROW_WORDS_PER_PLANE + 2 * q] = (uint32_t)__double2loint(val);
+                        w[z * ZROW_WORDS_PER_PLANE + 2 * q + 1] = (uint32_t)__double2hiint(val);
                     }
-                    const uint32_t at = zrow + (uint32_t)((h * HALF_PLANES + z) * ZROW_WORDS_PER_PLANE);
-                    tmem_st8(at, w8);
-                    tmem_st2(at + 8, w2);
-                }
+                tmem_st110(zrow + (uint32_t)(h * HALF_PLANES * ZROW_WORDS_PER_PLANE), w);
                 tmem_wait_st();
             }
             __syncthreads();          // shared memory is free: the other half (or the next group's first half) may land
@@ -264,6 +282,7 @@ static_assert(NCOMP * PS * PS * XSTAGE_PITCH * 8 <= F64_DATA_BYTES, "x-sweep sta
 constexpr int RING_SLOTS = 3;
 constexpr int RING_DOUBLES = RING_SLOTS * 2 * NCOMP * F64_THREADS;   // 7680
 static_assert((NCOMP * SLAB_VAR + RING_DOUBLES) * 8 <= F64_DATA_BYTES, "slab + ring fit");
+static_assert(SLAB_X * ZROW_WORDS_PER_PLANE == 110 && HALF_PLANES * ZROW_WORDS_PER_PLANE == 110, "tmem_st110");
 struct RingColSrc {
     const double* src[NCOMP];
     double* ring;                                                    // &ring[0][0][0][t]
@@ -345,24 +364,16 @@ hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restr
             {
                 const int yi = t & 15, k = t >> 4;
                 const double* rowp = buf + k * SLAB_PLANE + (yi + NG) * SLAB_X;
-#pragma unroll 1
-                for (int xs = 0; xs < SLAB_X; ++xs) {
-                    uint32_t w8[8], w2[2];
+                uint32_t w[SLAB_X * ZROW_WORDS_PER_PLANE];
+#pragma unroll
+                for (int xs = 0; xs < SLAB_X; ++xs)
 #pragma unroll
                     for (int q = 0; q < NCOMP; ++q) {
                         const double val = rowp[var_of(0, q) * SLAB_VAR + xs];
-                        if (q < 4) {
-                            w8[2 * q] = (uint32_t)__double2loint(val);
-                            w8[2 * q + 1] = (uint32_t)__double2hiint(val);
-                        } else {
-                            w2[0] = (uint32_t)__double2loint(val);
-                            w2[1] = (uint32_t)__double2hiint(val);
-                        }
+                        w[xs * ZROW_WORDS_PER_PLANE + 2 * q] = (uint32_t)__double2loint(val);
+                        w[xs * ZROW_WORDS_PER_PLANE + 2 * q + 1] = (uint32_t)__double2hiint(val);
                     }
-                    const uint32_t at = xrow + (uint32_t)((s * SLAB_X + xs) * ZROW_WORDS_PER_PLANE);
-                    tmem_st8(at, w8);
-                    tmem_st2(at + 8, w2);
-                }
+                tmem_st110(xrow + (uint32_t)(s * SLAB_X * ZROW_WORDS_PER_PLANE), w);
                 tmem_wait_st();
             }
             __syncthreads();          // the slab buffer is free again
