@@ -334,6 +334,21 @@ def run_ours(args):
     roofline_alu["peak_measured_tflops"] = peak_meas_tf
     roofline_alu["peak_measured_fma_per_clk_per_sm"] = peak_meas_lanes
     roofline_alu["frac_of_measured_peak"] = ach_tf / peak_meas_tf
+    # what the instruction mix of the march costs in steady state: clocks per warp-march and sub-partition
+    # slot with 1..4 warps per sub-partition, no loads, no barriers; and the cost of an FMA with three distinct registers
+    issue_probe = None
+    if rank == 0:
+        ffma3 = hydro.gamer_hydro_issue_probe(0, 4)
+        march = {ax: [hydro.gamer_hydro_issue_probe(i + 1, k) for k in (1, 2, 3, 4)] for i, ax in enumerate("xyz")}
+        # a group is 16 x-, 11 y-, 8 z-marches on 4 sub-partitions: with every slot filled at the 4-warp rate
+        packed = (16 * march["x"][3] + 11 * march["y"][3] + 8 * march["z"][3]) / 4.0
+        # the kernel's three phases run 4, 3 and 2 warps per sub-partition
+        phases = 4 * march["x"][3] + 3 * march["y"][2] + 2 * march["z"][1]
+        clk = peaks["sm_max_mhz"] * 1e6
+        issue_probe = dict(api="gamer_hydro_issue_probe", ffma_3_distinct_registers_clocks_per_instr=ffma3,
+                           clocks_per_warp_march_by_warps_per_subpartition=march,
+                           ns_per_group_if_every_slot_ran_at_the_4_warp_rate=packed / clk * 1e9 / n_sm,
+                           ns_per_group_sum_of_the_three_phases=phases / clk * 1e9 / n_sm)
     # the metric's roofline is the slower of the two bounds (north_star): FP32 at 51 ns/group vs HBM at 45 ns/group
     t_alu = FLOPS_PER_GROUP / (fp32_peak_tflops * 1e12)
     t_hbm = BYTES_PER_GROUP / (peaks["hbm_gbs"] * 1e9)
@@ -521,7 +536,7 @@ def run_ours(args):
                                 launch=info),
                     roofline=roofline, roofline_hbm=roofline_hbm, roofline_alu=roofline_alu,
                     cpu_baseline=cpu_baseline, cpu_baseline_1thread=cpu_1thread, e2e=e2e, gpu_launches=args.steps,
-                    clocks=clocks, backward=backward, config4=config4, failed=failed,
+                    clocks=clocks, backward=backward, issue_probe=issue_probe, config4=config4, failed=failed,
                     next3_ghost_fill=ghost_fill, next12_optional_outputs=optional_outputs, next4_f64=f64, next3_run_uniform=run_uniform,
                     parity_spot_check_max_rel=parity)
         print(json.dumps(line))

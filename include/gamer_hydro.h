@@ -154,6 +154,16 @@ GAMER_API int gamer_hydro_launch_info(long long n_groups, int* grid, int* block,
 GAMER_API int gamer_hydro_fp32_peak(int repeats, float* d_sink, double* tflops, double* lane_fma_per_clk_per_sm,
                           double sm_mhz);
 
+/* Measurement aid for DESIGN.md 7 (why the pass is bound by instruction issue and register-file reads), SYNCHRONOUS,
+ * allocates and frees its own few hundred KB of device memory; not part of the hydro path.
+ *   what = 0: *cycles = clocks one SM sub-partition needs per warp-wide FMA whose three source operands are three
+ *             different registers (an FMA with two reused operands takes 1.05), 4 warps per sub-partition;
+ *   what = 1, 2, 3: *cycles = clocks per warp-march (one warp, 32 rows of 22 cells, the production row march along x, y,
+ *             z) and sub-partition slot when warps_per_smsp = 1..4 warps per sub-partition run marches back to back
+ *             on a resident group with no loads and no barriers — the steady-state cost a schedule can at best reach.
+ * Values are means over the SMs of the current device, read from clock64 inside the kernels. */
+GAMER_API int gamer_hydro_issue_probe(int what, int warps_per_smsp, double* cycles);
+
 GAMER_API const char* gamer_last_error(void);   /* thread-local, static storage; "" if the last call on this thread succeeded */
 GAMER_API const char* gamer_version(void);      /* static string */
 

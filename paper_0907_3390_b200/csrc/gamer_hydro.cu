@@ -175,6 +175,67 @@ __global__ void __launch_bounds__(PEAK_THREADS) fp32_peak_kernel(float* __restri
     if (s == 123.456f) sink[0] = s;                                    // keeps the chains alive, never true in practice
 }
 
+// Issue-rate probes: what an SM sub-partition sustains on the instruction mix of this kernel.
+//   ffma3_probe_kernel: fused multiply-adds whose three source operands are three different registers that no
+//     neighbouring instruction shares (the register file delivers about two operands per clock to a sub-partition:
+//     such an FMA costs 1.5 issue slots, one with two reused operands costs 1).
+//   march_probe_kernel<D>: the production row march (rtvd_march.cuh, the sweep of hydro_kernel.cuh along axis D) back to
+//     back on k warps per sub-partition, in place on one resident group, no loads, no barriers: cycles per warp-march.
+constexpr int PROBE3_CHAINS = 16, PROBE3_ITERS = 2000;
+__global__ void __launch_bounds__(512, 1) ffma3_probe_kernel(float* __restrict__ sink, long long* __restrict__ cyc) {
+    float x[PROBE3_CHAINS], y[PROBE3_CHAINS], z[PROBE3_CHAINS];
+#pragma unroll
+    for (int i = 0; i < PROBE3_CHAINS; ++i) {
+        x[i] = threadIdx.x * 1e-3f + i;
+        y[i] = 1.0f + 1e-6f * (threadIdx.x + i);
+        z[i] = 1e-7f * (threadIdx.x + 3 * i);
+    }
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < PROBE3_ITERS; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < PROBE3_CHAINS; ++i) x[i] = fmaf(x[i], y[i], z[i]);
+    }
+    const long long t1 = clock64();
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < PROBE3_CHAINS; ++i) s += x[i] + y[i] + z[i];
+    if (s == 123.456f) sink[0] = s;
+    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned long long*>(&cyc[blockIdx.x]), (unsigned long long)(t1 - t0));
+}
+
+template <int D>
+__global__ void __launch_bounds__(gamer::BLOCK_THREADS, 1)
+march_probe_kernel(const float* __restrict__ in, gamer::GasConst gc, int k_per_smsp, int reps, long long* __restrict__ cyc,
+                   float* __restrict__ sink) {
+    using namespace gamer;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* smem = reinterpret_cast<float*>(smem_raw);
+    for (int i = threadIdx.x; i < GROUP_IN_FLOATS; i += blockDim.x) smem[i] = in[i];
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    NoGate nogate;
+    float speed = 0.f;
+    const long long t0 = clock64();
+    if (warp < 4 * k_per_smsp) {
+#pragma unroll 1
+        for (int r = 0; r < reps; ++r) {
+            // rows are shared between warps where a sweep has fewer than 512: same values, timing only
+            if (D == 0)
+                sweep<0, 0, NP, 0, NP, false, false, false, false>(smem, gc, nullptr, nullptr, speed, (32 * warp + lane) % 480, nogate);
+            else if (D == 1)
+                sweep<1, NG, PS, 0, NP, false, false, false, false>(smem, gc, nullptr, nullptr, speed, ((threadIdx.x % 352) & ~31) | lane, nogate);
+            else
+                sweep<2, NG, PS, NG, PS, false, false, false, false>(smem, gc, nullptr, nullptr, speed, threadIdx.x % 256, nogate);
+        }
+    }
+    const long long t1 = clock64();
+    if (lane == 0) atomicMax(reinterpret_cast<unsigned long long*>(&cyc[blockIdx.x]), (unsigned long long)(t1 - t0));
+    if (smem[12345] == 123.456f) sink[0] = smem[12345] + speed;
+}
+
 }  // namespace
 
 extern "C" {
@@ -494,6 +555,57 @@ int gamer_hydro_fp32_peak(int repeats, float* d_sink, double* tflops, double* la
     const double fma = (double)grid * PEAK_THREADS * PEAK_CHAINS * PEAK_ITERS;
     *tflops = 2.0 * fma / (best_ms * 1e-3) / 1e12;
     if (lane_fma_per_clk_per_sm) *lane_fma_per_clk_per_sm = sm_mhz > 0 ? fma / (best_ms * 1e-3) / (sm_mhz * 1e6) / sm : 0.0;
+    g_err[0] = '\0';
+    return GAMER_OK;
+}
+
+int gamer_hydro_issue_probe(int what, int warps_per_smsp, double* cycles) {
+    if (cycles == nullptr || what < 0 || what > 3 || warps_per_smsp < 1 || warps_per_smsp > 4)
+        return fail(GAMER_EINVAL, "issue_probe: what in 0..3, warps_per_smsp in 1..4, cycles non-NULL");
+    int sm_count = 0;
+    int rc = prepare(reinterpret_cast<const void*>(march_probe_kernel<0>), 17, gamer::SMEM_BYTES, &sm_count);
+    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(march_probe_kernel<1>), 18, gamer::SMEM_BYTES, &sm_count);
+    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(march_probe_kernel<2>), 19, gamer::SMEM_BYTES, &sm_count);
+    if (rc != GAMER_OK) return rc;
+    // one group of a smooth, physical, non-uniform state; a tiny dt/dh keeps it so over the in-place repetitions
+    std::vector<float> h(gamer::GROUP_IN_FLOATS);
+    unsigned int seed = 12345u;
+    for (int v = 0; v < gamer::NCOMP; ++v)
+        for (int i = 0; i < gamer::VAR_FLOATS; ++i) {
+            seed = seed * 1664525u + 1013904223u;
+            const float r = (float)(seed >> 8) * (1.0f / 16777216.0f);
+            h[(size_t)v * gamer::VAR_FLOATS + i] = v == 0 ? 1.f + 0.1f * r : (v == 4 ? 1.5f + 0.1f * r : 0.1f * (r - 0.5f));
+        }
+    float* d_in = nullptr;
+    long long* d_cyc = nullptr;
+    float* d_sink = nullptr;
+    cudaError_t e = cudaMalloc(&d_in, gamer::GROUP_IN_BYTES);
+    if (e == cudaSuccess) e = cudaMalloc(&d_cyc, (size_t)sm_count * sizeof(long long));
+    if (e == cudaSuccess) e = cudaMalloc(&d_sink, sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpy(d_in, h.data(), gamer::GROUP_IN_BYTES, cudaMemcpyHostToDevice);
+    const int reps = 20;
+    gamer::GasConst gc = make_const(0.01f, 1.0f, 5.0f / 3.0f);
+    std::vector<long long> c(sm_count);
+    for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {          // the first pass is a warm-up
+        e = cudaMemset(d_cyc, 0, (size_t)sm_count * sizeof(long long));
+        if (e != cudaSuccess) break;
+        if (what == 0) ffma3_probe_kernel<<<sm_count, 512>>>(d_sink, d_cyc);
+        else if (what == 1) march_probe_kernel<0><<<sm_count, gamer::BLOCK_THREADS, gamer::SMEM_BYTES>>>(d_in, gc, warps_per_smsp, reps, d_cyc, d_sink);
+        else if (what == 2) march_probe_kernel<1><<<sm_count, gamer::BLOCK_THREADS, gamer::SMEM_BYTES>>>(d_in, gc, warps_per_smsp, reps, d_cyc, d_sink);
+        else march_probe_kernel<2><<<sm_count, gamer::BLOCK_THREADS, gamer::SMEM_BYTES>>>(d_in, gc, warps_per_smsp, reps, d_cyc, d_sink);
+        e = cudaDeviceSynchronize();
+        if (e == cudaSuccess) e = cudaMemcpy(c.data(), d_cyc, (size_t)sm_count * sizeof(long long), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(d_in);
+    cudaFree(d_cyc);
+    cudaFree(d_sink);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(GAMER_ECUDA, "issue_probe: %s", cudaGetErrorString(e)); }
+    double mean = 0.0;
+    for (int i = 0; i < sm_count; ++i) mean += (double)c[i];
+    mean /= sm_count;
+    // what = 0: 4 warps per sub-partition (512 threads), cycles per warp instruction of one sub-partition;
+    // what = 1..3: cycles per warp-march and sub-partition slot
+    *cycles = what == 0 ? mean / (4.0 * PROBE3_ITERS * 4 * PROBE3_CHAINS) : mean / reps / warps_per_smsp;
     g_err[0] = '\0';
     return GAMER_OK;
 }

@@ -60,6 +60,8 @@ def lib():
         L.gamer_hydro_fp32_peak.restype = ci
         L.gamer_hydro_fp32_peak.argtypes = [ci, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                             ctypes.c_double]
+        L.gamer_hydro_issue_probe.restype = ci
+        L.gamer_hydro_issue_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
         L.gamer_last_error.restype = ctypes.c_char_p
         L.gamer_last_error.argtypes = []
         L.gamer_version.restype = ctypes.c_char_p
@@ -195,3 +197,10 @@ def gamer_hydro_launch_info(n_groups):
     g, b, s, r = (ctypes.c_int(0) for _ in range(4))
     _check(lib().gamer_hydro_launch_info(n_groups, ctypes.byref(g), ctypes.byref(b), ctypes.byref(s), ctypes.byref(r)))
     return dict(grid=g.value, block=b.value, smem_bytes=s.value, regs_per_thread=r.value)
+
+
+def gamer_hydro_issue_probe(what, warps_per_smsp=4):
+    """Measurement aid: clocks per 3-register FMA (what = 0) or per warp-march along x, y, z (1, 2, 3)."""
+    c = ctypes.c_double(0.0)
+    _check(lib().gamer_hydro_issue_probe(int(what), int(warps_per_smsp), ctypes.byref(c)))
+    return c.value

@@ -126,3 +126,11 @@ def test_oracle_and_product_do_not_import_each_other():
             src = open(os.path.join(ROOT, "oracle", fn)).read()
             assert "paper_0907_3390_b200" not in src.replace("paper_0907_3390_b200/csrc)", ""), fn
             assert "gamer_hydro.h" not in src and "rtvd_march" not in src, fn
+
+
+def test_issue_probe_rejects_bad_arguments_without_a_device():
+    import ctypes
+    c = ctypes.c_double(0.0)
+    assert hydro.lib().gamer_hydro_issue_probe(4, 1, ctypes.byref(c)) == hydro.GAMER_EINVAL
+    assert hydro.lib().gamer_hydro_issue_probe(1, 5, ctypes.byref(c)) == hydro.GAMER_EINVAL
+    assert hydro.lib().gamer_hydro_issue_probe(1, 1, None) == hydro.GAMER_EINVAL

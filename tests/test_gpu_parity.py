@@ -269,3 +269,15 @@ def test_runs_on_a_side_stream():
         gpu = gpu_advance(c["inp"], c["dt"], c["dh"], c["gamma"], stream=s)
     o32 = oracle.hydro_advance(c["inp"], c["dt"], c["dh"], c["gamma"])
     assert W.parity_error(gpu, o32, c["gamma"])["max_rel"] <= TOL32
+
+
+@pytest.mark.gpu
+def test_issue_probe_reports_plausible_clock_counts():
+    """The measurement aid behind DESIGN.md 7: a 3-register FMA costs more than one issue slot and less than two; a
+    warp-march (about 2 700 instructions) costs between 2 700 and 4 500 clocks and gets cheaper per slot with more warps."""
+    f3 = hydro.gamer_hydro_issue_probe(0, 4)
+    assert 1.2 <= f3 <= 2.0, f3
+    for what in (1, 2, 3):
+        c1, c4 = hydro.gamer_hydro_issue_probe(what, 1), hydro.gamer_hydro_issue_probe(what, 4)
+        assert 2700 <= c4 <= c1 <= 4500, (what, c1, c4)
+
