@@ -68,8 +68,9 @@ struct SmemSink {
     float* fptr[NCOMP];      // &face_flux[g][d][0][var(q)][b][a], or unused
     bool face_row;
     float held[NCOMP];
-    template <int ODD>
+    template <int P>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
+        constexpr int ODD = P & 1;
         if (STRIDE == 1 && !GAMER_X32) {
             if (ODD) {
                 if (j == NG) {
@@ -112,18 +113,26 @@ struct FinalSink {
     float gm1, ggm1;
     float speed;             // running max of c_s + max|v_i|
     float held[NCOMP];
-    template <int ODD>
+    float h1[TO_GLOBAL && STRIDE == 1 ? NCOMP : 1], h2[TO_GLOBAL && STRIDE == 1 ? NCOMP : 1];
+    template <int P>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
+        constexpr int ODD = P & 1;
         if (TO_GLOBAL && STRIDE == 1) {
-            // backward pass, last sweep along x: a thread owns the 16 contiguous cells of its output row (64 B, aligned);
-            // interior cells i = j - 3 go out in pairs (i even, i + 1) as 64-bit stores: the odd padded cell waits
-            if (ODD) {
+            // backward pass, last sweep along x (PHASE4 march): a thread owns the 16 contiguous cells of its output row
+            // (64 B, aligned) and sends them off four at a time, as 128-bit stores; P = position in the group of four
+            if (P == 3) {
 #pragma unroll
                 for (int k = 0; k < NCOMP; ++k) held[k] = u[k];
+            } else if (P == 0) {
+#pragma unroll
+                for (int k = 0; k < NCOMP; ++k) h1[k] = u[k];
+            } else if (P == 1) {
+#pragma unroll
+                for (int k = 0; k < NCOMP; ++k) h2[k] = u[k];
             } else {
 #pragma unroll
                 for (int k = 0; k < NCOMP; ++k)
-                    *reinterpret_cast<float2*>(dst[k] + (j - 1 - NG)) = make_float2(held[k], u[k]);
+                    *reinterpret_cast<float4*>(dst[k] + (j - 3 - NG)) = make_float4(held[k], h1[k], h2[k], u[k]);
             }
         } else if (TO_GLOBAL) {
 #pragma unroll
@@ -246,7 +255,7 @@ __device__ __forceinline__ void sweep(float* smem, const GasConst& gc, float* __
         sink.gm1 = gc.gm1;
         sink.ggm1 = gc.ggm1;
         sink.speed = speed;
-        rtvd_march<STRIDE, WANT_FACE>(src, gc, sink, gate);
+        rtvd_march<STRIDE, WANT_FACE, LAST_TO_GLOBAL && D == 0>(src, gc, sink, gate);
         speed = sink.speed;
     }
 }
@@ -510,6 +519,23 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             __syncthreads();
             // last sweep: along x, in place; then a coalesced 128-bit copy-out of the interior, chunk by chunk, each
             // chunk's planes handed to the bulk copies of the next group as soon as they have been read
+#ifndef GAMER_BWD_DIRECT
+#define GAMER_BWD_DIRECT 1
+#endif
+#if GAMER_BWD_DIRECT
+            // last sweep: along x, every thread sends its row to HBM itself, four cells per 128-bit store (lanes 64 B
+            // apart: half of every sector written per store, the other half by the next one); no copy-out, and all the
+            // interior planes are handed to the next group's bulk copies at once
+            sweep<0, NG, PS, NG, PS, true, true, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
+                                                                        nogate);
+            if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);
+            __syncthreads();
+            if (threadIdx.x == 0 && has_next) {
+                fence_proxy_async();
+                for (int c = 1; c < N_BCHUNK - 1; ++c) load_bchunk(smem, ctl, in_next, c);
+            }
+            continue;
+#endif
             sweep<0, NG, PS, NG, PS, true, false, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
                                                                          nogate);
             if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);

@@ -185,7 +185,9 @@ __device__ __forceinline__ T limited(T base, T a, T b) {
 // cannot fill the issue slots: latching cost 5 registers and one drain step per row and gained 3.4 %.
 // Steps 0..7 fill the pipeline (PH = n, statically pruned); steps 8..21 are identical and run as a rolled loop
 // (PH = 7), so that the code stays resident in the instruction cache; a last half step drains cell 18.
-template <bool WANT_FACE, class Sink, class T = float>
+// PHASE4: the steady loop is written out in bodies of two pairs and Sink::cell<P> receives P = (j - 4) mod 4 — the position
+// of the cell in a group of four, for a sink that collects four cells into one 128-bit store; otherwise P = j mod 2.
+template <bool WANT_FACE, class Sink, class T = float, bool PHASE4 = false>
 struct RowMarch {
     T u1[NCOMP], u2[NCOMP], u3[NCOMP], u4[NCOMP];   // u_{n-1} .. u_{n-4} (the originals, kept for Eqs.13-14)
     T sig1, cp1, P1, Pv1;                  // 1 - 2 q c, q (c+v), q P, q P v of cell n-1
@@ -197,7 +199,7 @@ struct RowMarch {
     T fh_prev[NCOMP];                      // 2 F^h through (m-3|m-2)
 
     // stage B of step n: everything that follows from the midpoint state of cell m = n-2; new value of cell j = n-4
-    template <int PH, int ODD>
+    template <int PH, int ODD, int Q = 0>
     __device__ __forceinline__ void stage_b(int n, const GasConstT<T>& gc, Sink& sink) {
         if (PH >= 3) {
             T gr2[NCOMP], gl2[NCOMP];
@@ -234,7 +236,7 @@ struct RowMarch {
                         T un[NCOMP];
 #pragma unroll
                         for (int k = 0; k < NCOMP; ++k) un[k] = fma_rn(-gc.kh, fh[k] - fh_prev[k], u4[k]);
-                        sink.template cell<ODD>(n - 4, un);
+                        sink.template cell<2 * Q + ODD>(n - 4, un);
                     }
 #pragma unroll
                     for (int k = 0; k < NCOMP; ++k) fh_prev[k] = fh[k];
@@ -278,15 +280,15 @@ struct RowMarch {
         cp1 = h.cp; P1 = h.P; Pv1 = h.Pv; sig1 = h.sig;
     }
 
-    template <int PH0, int PH1, class Src, class Gate>
+    template <int PH0, int PH1, int Q = 0, class Src, class Gate>
     __device__ __forceinline__ void pair(Src& src, int n, const GasConstT<T>& gc, Sink& sink, Gate& gate) {
         T ua[NCOMP], ub[NCOMP];
         gate.acquire(n);
         src.load(n, ua, ub);
         gate.release(n);
-        stage_b<PH0, 0>(n, gc, sink);           // n is even: j = n-4 is even
+        stage_b<PH0, 0, Q>(n, gc, sink);        // n is even: j = n-4 is even
         stage_a<PH0>(ua, gc);
-        stage_b<PH1, 1>(n + 1, gc, sink);
+        stage_b<PH1, 1, Q>(n + 1, gc, sink);
         stage_a<PH1>(ub, gc);
     }
 
@@ -295,6 +297,17 @@ struct RowMarch {
         pair<0, 1>(src, 0, gc, sink, gate);
         pair<2, 3>(src, 2, gc, sink, gate);
         pair<4, 5>(src, 4, gc, sink, gate);
+        if (PHASE4) {
+            pair<6, 7, 1>(src, 6, gc, sink, gate);          // cell 3 at step 7: P = 3, the first of a group of four
+#pragma unroll 1
+            for (int n = 8; n < NP - 2; n += 4) {
+                pair<7, 7, 0>(src, n, gc, sink, gate);      // cells n-4, n-3: P = 0, 1
+                pair<7, 7, 1>(src, n + 2, gc, sink, gate);  // cells n-2, n-1: P = 2 (the group is complete), 3
+            }
+            pair<7, 7, 0>(src, NP - 2, gc, sink, gate);     // cells 16, 17
+            stage_b<7, 0, 1>(NP, gc, sink);                 // drain: cell 18, P = 2
+            return;
+        }
         pair<6, 7>(src, 6, gc, sink, gate);
         // pairs of cells per loop body: the fp64 step is 2.5 x as long, so its body is kept shorter
         constexpr int UNROLL = sizeof(T) == 8 ? GAMER_MARCH_UNROLL_F64 : MARCH_UNROLL;
@@ -331,10 +344,10 @@ struct NoGate {
     __device__ __forceinline__ void release(int) {}
 };
 
-template <int STRIDE, bool WANT_FACE, class Sink, class Gate>
+template <int STRIDE, bool WANT_FACE, bool PHASE4 = false, class Sink, class Gate>
 __device__ __forceinline__ void rtvd_march(const float* const (&src)[NCOMP], const GasConst& gc, Sink& sink,
                                            Gate& gate) {
-    RowMarch<WANT_FACE, Sink> m;
+    RowMarch<WANT_FACE, Sink, float, PHASE4> m;
     StrideSrc<STRIDE> s;
 #pragma unroll
     for (int k = 0; k < NCOMP; ++k) s.src[k] = src[k];
