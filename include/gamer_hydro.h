@@ -130,14 +130,18 @@ GAMER_API int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx
 
 /* NEXT-4 — one pass in DOUBLE precision (the paper switches to double for its convergence tests).
  * Same operation, layouts and error conventions as gamer_hydro_advance_ex with double arrays: d_in
- * [g][v][22][22][22] (425 920 B per group), d_out [g][v][16][16][16]; backward = 0 sweeps x,y,z, 1 sweeps z,y,x.
- * Reciprocals and square roots are accurate to about 1 ulp.  d_scratch: device scratch of
- * gamer_hydro_f64_scratch_doubles() doubles, 16-byte aligned, owned by the caller, not shared between concurrent calls
- * (one block per SM: the group does not fit in shared memory and the pass goes through it between sweeps).  No
- * optional outputs. */
+ * [g][v][22][22][22] (425 920 B per group), d_out [g][v][16][16][16]; backward = 0 sweeps x,y,z, 1 sweeps z,y,x;
+ * d_face_flux [g][3][3][5][16][16] and d_group_maxspeed [g] are the optional outputs of gamer_hydro_advance_ex in
+ * double (NULL = off).  Reciprocals and square roots are accurate to about 1 ulp.  A padded group does not fit in
+ * shared memory in double precision: the pass is cut into halves and the rows of the last sweep wait in tensor memory
+ * (DESIGN.md 8c); no device scratch is needed. */
+GAMER_API int gamer_hydro_advance_f64_ex(const double* d_in, double* d_out, long long n_groups, int ghost,
+                            double dt, double dh, double gamma, int backward, double* d_face_flux,
+                            double* d_group_maxspeed, void* stream);
+/* The same without optional outputs.  d_scratch is ignored (round 1 needed gamer_hydro_f64_scratch_doubles() doubles
+ * of device scratch; the function now returns 0) and may be NULL. */
 GAMER_API int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost,
                             double dt, double dh, double gamma, int backward, double* d_scratch, void* stream);
-/* Doubles of scratch gamer_hydro_advance_f64 needs on the current device; 0 (and an error message) without a device. */
 GAMER_API size_t gamer_hydro_f64_scratch_doubles(void);
 
 /* Launch geometry the library will use on the current device, for reporting: any pointer may be NULL.

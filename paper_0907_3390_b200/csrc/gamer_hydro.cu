@@ -55,7 +55,7 @@ KernelFn pick_kernel(bool backward, bool face, bool speed) {
 struct DeviceInfo {
     bool ready = false;
     int sm_count = 0;
-    bool attr_set[16] = {};
+    bool attr_set[32] = {};      // one flag per kernel key (prepare())
 };
 std::mutex g_mu;
 DeviceInfo g_dev[64];
@@ -458,41 +458,34 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     return GAMER_OK;
 }
 
-size_t gamer_hydro_f64_scratch_doubles(void) {
-    int dev = 0, sm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
-        (void)cudaGetLastError();
-        fail(GAMER_ECUDA, "no CUDA device");
-        return 0;
-    }
-    return (size_t)sm * gamer::F64_SCRATCH_DOUBLES;
-}
+size_t gamer_hydro_f64_scratch_doubles(void) { return 0; }      // round 1 passed rows through device memory; tensor memory now
 
-int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost, double dt, double dh,
-                            double gamma, int backward, double* d_scratch, void* stream) {
+int gamer_hydro_advance_f64_ex(const double* d_in, double* d_out, long long n_groups, int ghost, double dt, double dh,
+                               double gamma, int backward, double* d_face_flux, double* d_group_maxspeed, void* stream) {
     if (ghost != gamer::NG)
         return fail(GAMER_EUNSUPPORTED, "ghost = %d: the 7-point stencil of the scheme fixes ghost = 3", ghost);
     if (n_groups < 0) return fail(GAMER_EINVAL, "n_groups = %lld < 0", n_groups);
     if (!(dh > 0.0) || !(dt >= 0.0) || !(gamma > 1.0)) return fail(GAMER_EINVAL, "need dh > 0, dt >= 0, gamma > 1");
     if (backward != 0 && backward != 1) return fail(GAMER_EINVAL, "backward must be 0 or 1");
-    if (n_groups > 0 && (d_in == nullptr || d_out == nullptr || d_scratch == nullptr))
-        return fail(GAMER_EINVAL, "NULL input, output or scratch pointer");
-    if (!aligned16(d_in) || !aligned16(d_out) || !aligned16(d_scratch))
+    if (n_groups > 0 && (d_in == nullptr || d_out == nullptr)) return fail(GAMER_EINVAL, "NULL input or output pointer");
+    if (!aligned16(d_in) || !aligned16(d_out) || !aligned16(d_face_flux) || !aligned16(d_group_maxspeed))
         return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
     {
-        const void* ptr[2] = {d_in, d_out};
-        const size_t bytes[2] = {(size_t)n_groups * gamer::GROUP_IN_FLOATS * sizeof(double),
-                                 (size_t)n_groups * gamer::GROUP_OUT_FLOATS * sizeof(double)};
-        const int rc0 = check_disjoint(ptr, bytes, 2);
+        const size_t n = (size_t)n_groups, db = sizeof(double);
+        const void* ptr[4] = {d_in, d_out, d_face_flux, d_group_maxspeed};
+        const size_t bytes[4] = {n * gamer::GROUP_IN_FLOATS * db, n * gamer::GROUP_OUT_FLOATS * db,
+                                 n * gamer::GROUP_FACE_FLOATS * db, n * db};
+        const int rc0 = check_disjoint(ptr, bytes, 4);
         if (rc0 != GAMER_OK) return rc0;
     }
     g_err[0] = '\0';
     if (n_groups == 0) return GAMER_OK;
     int sm_count = 0;
-    using F64Fn = void (*)(const double*, double*, long long, gamer::GasConstT<double>, double*);
-    F64Fn fn = backward ? gamer::hydro_advance_f64_backward_kernel : gamer::hydro_advance_f64_kernel;
-    const int rc = prepare(reinterpret_cast<const void*>(fn), backward ? 10 : 9, gamer::F64_SMEM_BYTES, &sm_count);
+    using F64Fn = void (*)(const double*, double*, long long, gamer::GasConstT<double>, double*, double*);
+    const bool opt = d_face_flux != nullptr || d_group_maxspeed != nullptr;
+    F64Fn fn = backward ? (opt ? gamer::hydro_advance_f64_backward_kernel<true> : gamer::hydro_advance_f64_backward_kernel<false>)
+                        : (opt ? gamer::hydro_advance_f64_kernel<true> : gamer::hydro_advance_f64_kernel<false>);
+    const int rc = prepare(reinterpret_cast<const void*>(fn), (backward ? 10 : 9) + (opt ? 11 : 0), gamer::F64_SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
     gamer::GasConstT<double> gc;
     const double k = dt / dh;
@@ -506,10 +499,16 @@ int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_group
     gc.kq_sg = gc.kq * gc.sg;
     const int grid = (int)(n_groups < (long long)sm_count ? n_groups : (long long)sm_count);
     fn<<<grid, gamer::F64_THREADS, gamer::F64_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(d_in, d_out, n_groups, gc,
-                                                                                            d_scratch);
+                                                                                            d_face_flux, d_group_maxspeed);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
     return GAMER_OK;
+}
+
+int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost, double dt, double dh,
+                            double gamma, int backward, double* d_scratch, void* stream) {
+    (void)d_scratch;          // no longer used (any value, NULL included)
+    return gamer_hydro_advance_f64_ex(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward, nullptr, nullptr, stream);
 }
 
 int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread) {

@@ -35,7 +35,7 @@ constexpr int BWD_CHUNK_VAR = BWD_CHUNK_PLANES * NP * NP;            // 3872
 constexpr int FWD_SCRATCH_DOUBLES = NCOMP * ZBUF_VAR;                // 28 160 per CTA (forward pass)
 constexpr int F64_SCRATCH_DOUBLES = BWD_SCRATCH_DOUBLES;             // what the caller provides per CTA
 constexpr int F64_DATA_BYTES = FWD_SCRATCH_DOUBLES * 8;              // 225 280 (>= 5 * 5324 * 8 = 212 960)
-constexpr int F64_SMEM_BYTES = F64_DATA_BYTES + 64;
+constexpr int F64_SMEM_BYTES = F64_DATA_BYTES + 128;     // + mbarrier, TMEM base address, 8 doubles of reduction scratch
 
 
 // ---- tensor memory (tcgen05) as per-thread row storage ----------------------------------------------------------
@@ -133,35 +133,82 @@ struct SrcF64 {
 };
 
 // Writes updated cell j to dst[k] + (j - J0) * STRIDE (in place in shared memory: J0 = 0; to `out`: J0 = NG).
-template <int STRIDE, int J0>
+// WANT_FACE: the time-centred fluxes through the three patch-boundary planes go to fptr[k] + p * 5 * 256 if this row is
+// an interior one (the layout of gamer_hydro.h: face_flux[g][d][p][v][b][a]).  WANT_SPEED: Eq.30 on
+// every updated cell of the last sweep, running maximum in `speed`.
+template <int STRIDE, int J0, bool WANT_FACE = false, bool WANT_SPEED = false>
 struct SinkF64 {
     double* dst[NCOMP];
+    double* fptr[WANT_FACE ? NCOMP : 1];
+    bool face_row;
+    double ggm1, speed;
     template <int ODD>
     __device__ __forceinline__ void cell(int j, const double (&u)[NCOMP]) {
 #pragma unroll
         for (int k = 0; k < NCOMP; ++k) dst[k][(j - J0) * STRIDE] = u[k];
+        if (WANT_SPEED) {
+            const double rinv = rcp_fast(u[0]);
+            double q = u[2] * u[2];
+            q = fma(u[3], u[3], q);
+            q = fma(u[1], u[1], q);
+            const double eint = fma(-q, 0.5 * rinv, u[4]);
+            const double cs = sqrt_fast((ggm1 * eint) * rinv);
+            const double vm = fmax(fmax(fabs(u[1]), fabs(u[2])), fabs(u[3])) * rinv;
+            speed = fmax(speed, cs + vm);
+        }
     }
-    __device__ __forceinline__ void face(int, const double (&)[NCOMP]) {}
+    __device__ __forceinline__ void face(int p, const double (&f)[NCOMP]) {
+        if (WANT_FACE && face_row) {
+#pragma unroll
+            for (int k = 0; k < NCOMP; ++k) fptr[WANT_FACE ? k : 0][p * (NCOMP * PS * PS)] = f[k];
+        }
+    }
 };
 
-template <int STRIDE, int J0>
+// &face_flux[g][D][0][var(q)][b][a] for row-local component q of a sweep along D (b, a: interior transverse indices)
+template <int D>
+__device__ __forceinline__ double* face_ptr(double* face_g, int q, int b, int a) {
+    return face_g + ((D * 3) * NCOMP + var_of(D, q)) * (PS * PS) + b * PS + a;
+}
+
+// In-place (or to `dst`) march of one row; D = sweep axis, (b, a) = interior transverse indices of the row for the face
+// fluxes (any value if face_g is NULL or the row is not an interior one: face_row = false).
+template <int STRIDE, int J0, int D, bool WANT_FACE>
 __device__ __forceinline__ void march_f64(double* const (&row)[NCOMP], double* const (&dst)[NCOMP],
-                                          const GasConstT<double>& gc) {
+                                          const GasConstT<double>& gc, double* face_g, bool face_row, int b, int a) {
     SrcF64<STRIDE> src;
-    SinkF64<STRIDE, J0> sink;
+    SinkF64<STRIDE, J0, WANT_FACE, false> sink;
 #pragma unroll
     for (int k = 0; k < NCOMP; ++k) {
         src.src[k] = row[k];
         sink.dst[k] = dst[k];
+        if (WANT_FACE) sink.fptr[k] = face_ptr<D>(face_g, k, b, a);
     }
+    sink.face_row = WANT_FACE && face_row && face_g != nullptr;
     NoGate gate;
-    RowMarch<false, decltype(sink), double> m;
+    RowMarch<WANT_FACE, decltype(sink), double> m;
     m.run(src, gc, sink, gate);
 }
 
+// Block maximum of the per-thread CFL speeds -> *dst (one double per group).  `red`: 8 doubles of shared memory.
+__device__ __forceinline__ void block_max_f64(double v, double* red, double* dst) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double m = red[0];
+        for (int w = 1; w < F64_THREADS / 32; ++w) m = fmax(m, red[w]);
+        *dst = m;
+    }
+}
+
+// WANT_OPT: the optional outputs of gamer_hydro_advance_f64_ex (either pointer may still be NULL): face_flux
+// [g][3][3][5][16][16] and group_maxspeed[g], as in the fp32 kernel.
+template <bool WANT_OPT>
 __global__ void __launch_bounds__(F64_THREADS, 1)
 hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out, long long n_groups,
-                         GasConstT<double> gc, double* __restrict__ /*scratch: the backward pass uses it*/) {
+                         GasConstT<double> gc, double* __restrict__ face_flux, double* __restrict__ group_maxspeed) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* buf = reinterpret_cast<double*>(smem_raw);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + F64_DATA_BYTES);
@@ -187,6 +234,7 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
         const double* in_g = in + g * (long long)GROUP_IN_FLOATS;
         const long long gn = g + gridDim.x;
+        double* face_g = WANT_OPT && face_flux != nullptr ? face_flux + g * (long long)GROUP_FACE_FLOATS : nullptr;
         for (int h = 0; h < 2; ++h) {
             // ---- planes 11h .. 11h+10 of all variables are on their way into shared memory (issued earlier) -------
 #if GAMER_F64_PREFETCH
@@ -200,7 +248,9 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
                 double* row[NCOMP];
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) row[q] = buf + var_of(0, q) * HALF_VAR + t * NP;
-                march_f64<1, 0>(row, row, gc);
+                const int y = t % NP, z = h * HALF_PLANES + t / NP;
+                march_f64<1, 0, 0, WANT_OPT>(row, row, gc, face_g, y >= NG && y < NG + PS && z >= NG && z < NG + PS, z - NG,
+                                             y - NG);
             }
             __syncthreads();
             // ---- y sweep: x = 3..18, 11 planes, in place -------------------------------------------------------
@@ -209,7 +259,8 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
                 double* row[NCOMP];
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) row[q] = buf + var_of(1, q) * HALF_VAR + z * (NP * NP) + x;
-                march_f64<NP, 0>(row, row, gc);
+                const int zz = h * HALF_PLANES + z;
+                march_f64<NP, 0, 1, WANT_OPT>(row, row, gc, face_g, zz >= NG && zz < NG + PS, zz - NG, x - NG);
             }
             __syncthreads();
             // ---- every z thread parks the cells of its column in these planes in tensor memory -------------------
@@ -247,12 +298,22 @@ hydro_advance_f64_kernel(const double* __restrict__ in, double* __restrict__ out
             for (int q = 0; q < NCOMP; ++q) dst[q] = out_g + var_of(2, q) * (PS * PS * PS) + y * PS + x;
             TmemRowSrc src;
             src.taddr = zrow;
-            SinkF64<PS * PS, NG> sink;
+            SinkF64<PS * PS, NG, WANT_OPT, WANT_OPT> sink;
 #pragma unroll
-            for (int q = 0; q < NCOMP; ++q) sink.dst[q] = dst[q];
+            for (int q = 0; q < NCOMP; ++q) {
+                sink.dst[q] = dst[q];
+                if (WANT_OPT) sink.fptr[q] = face_ptr<2>(face_g, q, y, x);
+            }
+            sink.face_row = face_g != nullptr;
+            sink.ggm1 = gc.ggm1;
+            sink.speed = 0.0;
             NoGate gate;
-            RowMarch<false, decltype(sink), double> m;
+            RowMarch<WANT_OPT, decltype(sink), double> m;
             m.run(src, gc, sink, gate);
+            if (WANT_OPT && group_maxspeed != nullptr) {
+                block_max_f64(sink.speed, reinterpret_cast<double*>(smem_raw + F64_DATA_BYTES + 32) , group_maxspeed + g);
+                __syncthreads();          // `red` is reused by the next group
+            }
         }
         // no barrier: the next copy into tensor memory is by the same thread, after its own march
     }
@@ -315,9 +376,11 @@ struct RingColSrc {
     }
 };
 
+template <bool WANT_OPT>
 __global__ void __launch_bounds__(F64_THREADS, 1)
 hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restrict__ out, long long n_groups,
-                                  GasConstT<double> gc, double* __restrict__ /*scratch: unused since round 2*/) {
+                                  GasConstT<double> gc, double* __restrict__ face_flux,
+                                  double* __restrict__ group_maxspeed) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* buf = reinterpret_cast<double*>(smem_raw);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem_raw + F64_DATA_BYTES + 16);
@@ -332,20 +395,24 @@ hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restr
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
         const double* in_g = in + g * (long long)GROUP_IN_FLOATS;
         const long long gn = g + gridDim.x;
+        double* face_g = WANT_OPT && face_flux != nullptr ? face_flux + g * (long long)GROUP_FACE_FLOATS : nullptr;
         for (int s = 0; s < 2; ++s) {
             // ---- z sweep of the slab: 22 x 11 rows (y, xs), device memory -> shared memory (interior planes) ---------
             if (t < NP * SLAB_X) {
                 const int y = t / SLAB_X, xs = t - y * SLAB_X;
                 RingColSrc src;
                 src.ring = buf + NCOMP * SLAB_VAR + t;
-                SinkF64<SLAB_PLANE, NG> sink;
+                SinkF64<SLAB_PLANE, NG, WANT_OPT, false> sink;
+                const int x = s * SLAB_X + xs;
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) {
-                    src.src[q] = in_g + var_of(2, q) * VAR_FLOATS + y * NP + s * SLAB_X + xs;
+                    src.src[q] = in_g + var_of(2, q) * VAR_FLOATS + y * NP + x;
                     sink.dst[q] = buf + var_of(2, q) * SLAB_VAR + t;
+                    if (WANT_OPT) sink.fptr[q] = face_ptr<2>(face_g, q, y - NG, x - NG);
                 }
+                sink.face_row = face_g != nullptr && y >= NG && y < NG + PS && x >= NG && x < NG + PS;
                 NoGate gate;
-                RowMarch<false, decltype(sink), double> m;
+                RowMarch<WANT_OPT, decltype(sink), double> m;
                 m.run(src, gc, sink, gate);
             } else if (t == F64_THREADS - 1 && s == 1 && gn < n_groups) {
                 bulk_prefetch_l2(in + gn * (long long)GROUP_IN_FLOATS, GROUP_IN_FLOATS * 8);
@@ -357,7 +424,8 @@ hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restr
                 double* row[NCOMP];
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) row[q] = buf + var_of(1, q) * SLAB_VAR + k * SLAB_PLANE + xs;
-                march_f64<SLAB_X, 0>(row, row, gc);
+                const int x = s * SLAB_X + xs;
+                march_f64<SLAB_X, 0, 1, WANT_OPT>(row, row, gc, face_g, x >= NG && x < NG + PS, k, x - NG);
             }
             __syncthreads();
             // ---- every x-row owner parks the slab's cells of its row in tensor memory ----------------------------------
@@ -386,12 +454,20 @@ hydro_advance_f64_backward_kernel(const double* __restrict__ in, double* __restr
             const int yi = t & 15, k = t >> 4;
             TmemRowSrc src;
             src.taddr = xrow;
-            SinkF64<XSTAGE_PITCH, NG> sink;
+            SinkF64<XSTAGE_PITCH, NG, WANT_OPT, WANT_OPT> sink;
 #pragma unroll
-            for (int q = 0; q < NCOMP; ++q) sink.dst[q] = buf + ((var_of(0, q) * PS + k) * PS) * XSTAGE_PITCH + yi;
+            for (int q = 0; q < NCOMP; ++q) {
+                sink.dst[q] = buf + ((var_of(0, q) * PS + k) * PS) * XSTAGE_PITCH + yi;
+                if (WANT_OPT) sink.fptr[q] = face_ptr<0>(face_g, q, k, yi);
+            }
+            sink.face_row = face_g != nullptr;
+            sink.ggm1 = gc.ggm1;
+            sink.speed = 0.0;
             NoGate gate;
-            RowMarch<false, decltype(sink), double> m;
+            RowMarch<WANT_OPT, decltype(sink), double> m;
             m.run(src, gc, sink, gate);
+            if (WANT_OPT && group_maxspeed != nullptr)
+                block_max_f64(sink.speed, reinterpret_cast<double*>(smem_raw + F64_DATA_BYTES + 32), group_maxspeed + g);
         }
         __syncthreads();
         {

@@ -53,6 +53,8 @@ def lib():
         L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
         L.gamer_hydro_advance_f64.restype = ci
         L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp]
+        L.gamer_hydro_advance_f64_ex.restype = ci
+        L.gamer_hydro_advance_f64_ex.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp, vp]
         L.gamer_hydro_f64_scratch_doubles.restype = ctypes.c_size_t
         L.gamer_hydro_f64_scratch_doubles.argtypes = []
         L.gamer_hydro_launch_info.restype = ci
@@ -181,6 +183,16 @@ def gamer_hydro_advance_f64(d_in, d_out, n_groups, ghost, dt, dh, gamma, d_scrat
     """One pass in double precision; d_scratch: gamer_hydro_f64_scratch_doubles() doubles."""
     rc = lib().gamer_hydro_advance_f64(_ptr(d_in), _ptr(d_out), n_groups, ghost, dt, dh, gamma, int(backward),
                                        _ptr(d_scratch), _stream_ptr(stream))
+    if check:
+        _check(rc)
+    return rc
+
+
+def gamer_hydro_advance_f64_ex(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward=0, d_face_flux=None,
+                               d_group_maxspeed=None, stream=None, check=True):
+    """One pass in double precision with the optional outputs (face fluxes, per-group CFL speed) in double."""
+    rc = lib().gamer_hydro_advance_f64_ex(_ptr(d_in), _ptr(d_out), n_groups, ghost, dt, dh, gamma, int(backward),
+                                          _ptr(d_face_flux), _ptr(d_group_maxspeed), _stream_ptr(stream))
     if check:
         _check(rc)
     return rc

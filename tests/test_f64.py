@@ -22,7 +22,9 @@ def test_f64_argument_validation_needs_no_device():
     a16 = (ctypes.addressof(buf) + 15) & ~15
     assert L.gamer_hydro_advance_f64(a16, a16, 1, 2, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EUNSUPPORTED
     assert L.gamer_hydro_advance_f64(a16, a16, -1, 3, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.4, 0, None, None) == hydro.GAMER_EINVAL      # scratch
+    assert L.gamer_hydro_advance_f64(None, a16, 1, 3, 0.1, 1.0, 1.4, 0, None, None) == hydro.GAMER_EINVAL       # NULL input
+    assert L.gamer_hydro_advance_f64_ex(a16, a16 + 4259200, 1, 3, 0.1, 1.0, 1.4, 0, a16 + 8, None, None) == hydro.GAMER_EINVAL   # face alignment
+    assert L.gamer_hydro_advance_f64_ex(a16, a16 + 4259200, 1, 3, 0.1, 1.0, 1.4, 0, a16 + 16, None, None) == hydro.GAMER_EINVAL  # face overlaps in
     assert L.gamer_hydro_advance_f64(a16, a16 + 8, 1, 3, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL    # alignment
     assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 0.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL
     assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.0, 0, a16, None) == hydro.GAMER_EINVAL
@@ -130,3 +132,39 @@ def test_f64_acoustic_wave_converges_at_second_order_on_the_gpu():
     slopes = [np.log2(e[i + 1] / e[i]) for i in range(2)]
     assert all(-2.6 <= s <= -1.5 for s in slopes), (e, slopes)
     assert e[2] < 0.02, e
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("backward", [0, 1])
+def test_f64_optional_outputs(backward):
+    """Face fluxes and the per-group CFL speed (:418-426) of the double-precision pass against
+    the fp64 oracle: 350 different groups of config 3, so that every persistent CTA takes two or three in a row; the
+    fluxes per element at the scale of the cells next to the interface (the fp32 test's metric) to 1e-11; and the
+    optional outputs do not change the main one."""
+    import torch
+    from test_gpu_parity import face_flux_local_scale
+    rng = np.random.default_rng(7 + backward)
+    c = W.config3()
+    idx = rng.permutation(c["inp"].shape[0])[:350]
+    inp = np.ascontiguousarray(c["inp"][idx]).astype(np.float64)
+    n = inp.shape[0]
+    d_in = torch.from_numpy(inp).cuda()
+    d_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float64, device="cuda")
+    d_face = torch.full((n, 3, 3, 5, 16, 16), float("nan"), dtype=torch.float64, device="cuda")
+    d_speed = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
+    hydro.gamer_hydro_advance_f64_ex(d_in, d_out, n, 3, c["dt"], c["dh"], c["gamma"], backward, d_face, d_speed)
+    torch.cuda.synchronize()
+    o_out, o_face, o_speed = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], backward=backward, dtype=np.float64,
+                                                  want_face_flux=True, want_maxspeed=True, n_threads=8)
+    out, face, speed = d_out.cpu().numpy(), d_face.cpu().numpy(), d_speed.cpu().numpy()
+    assert W.parity_error(out, o_out, c["gamma"])["max_rel"] <= TOL
+    np.testing.assert_allclose(speed, o_speed, rtol=1e-12)
+    assert np.isfinite(face).all()
+    err = np.abs(face - o_face) / face_flux_local_scale(inp, c["gamma"])
+    assert err.max() <= TOL, (err.max(), np.unravel_index(int(np.argmax(err)), err.shape))
+    assert np.array_equal(out, gpu_advance_f64(inp, c["dt"], c["dh"], c["gamma"], backward))
+    # only one of the two
+    d_speed.fill_(float("nan"))
+    hydro.gamer_hydro_advance_f64_ex(d_in, d_out, n, 3, c["dt"], c["dh"], c["gamma"], backward, None, d_speed)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(d_speed.cpu().numpy(), o_speed, rtol=1e-12)
