@@ -17,6 +17,7 @@
 #include <cstdint>
 
 #include "hydro_kernel.cuh"
+#include "tmem_rows.cuh"
 
 #ifndef GAMER_F64_PREFETCH
 #define GAMER_F64_PREFETCH 1
@@ -37,67 +38,6 @@ constexpr int F64_SCRATCH_DOUBLES = BWD_SCRATCH_DOUBLES;             // what the
 constexpr int F64_DATA_BYTES = FWD_SCRATCH_DOUBLES * 8;              // 225 280 (>= 5 * 5324 * 8 = 212 960)
 constexpr int F64_SMEM_BYTES = F64_DATA_BYTES + 128;     // + mbarrier, TMEM base address, 8 doubles of reduction scratch
 
-
-// ---- tensor memory (tcgen05) as per-thread row storage ----------------------------------------------------------
-// 32x32b shape: thread i of a warp accesses lane (32 * (warp % 4) + i), N consecutive 32-bit columns from the address.
-__device__ __forceinline__ void tmem_alloc_all(uint32_t* smem_slot) {        // one warp; writes the base address
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_slot)), "r"(512u)
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc_all(uint32_t taddr) {           // the same warp
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(512u) : "memory");
-}
-__device__ __forceinline__ void tmem_st2(uint32_t taddr, const uint32_t (&r)[2]) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
-}
-__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8]) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]),
-                 "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
-                 : "memory");
-}
-__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t* r) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]),
-                 "r"(r[3])
-                 : "memory");
-}
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-                 : "memory");
-}
-// One slab of a row, 11 cells x 5 variables x 2 words = 110 consecutive columns, in six instructions: a tcgen05.st costs
-// the same few dozen cycles of the SM's tensor-memory port whatever its width (22 narrow stores per row took 13 % of
-// the kernel).
-__device__ __forceinline__ void tmem_st110(uint32_t taddr, const uint32_t (&w)[110]) {
-    tmem_st32(taddr, w);
-    tmem_st32(taddr + 32, w + 32);
-    tmem_st32(taddr + 64, w + 64);
-    {
-        const uint32_t t8[8] = {w[96], w[97], w[98], w[99], w[100], w[101], w[102], w[103]};
-        tmem_st8(taddr + 96, t8);
-    }
-    tmem_st4(taddr + 104, w + 104);
-    {
-        const uint32_t t2[2] = {w[108], w[109]};
-        tmem_st2(taddr + 108, t2);
-    }
-}
-__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
-                 : "r"(taddr)
-                 : "memory");
-}
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-        : "r"(taddr)
-        : "memory");
-}
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 constexpr int ZROW_WORDS_PER_PLANE = 2 * NCOMP;                      // 10 columns: one cell, five doubles
 constexpr int ZROW_COLS = NP * ZROW_WORDS_PER_PLANE;                 // 220 columns per z row
