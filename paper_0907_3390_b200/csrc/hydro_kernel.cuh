@@ -4,10 +4,10 @@
 //   H0  the padded group (212 960 B, contiguous in HBM) is bulk-copied into shared memory with cp.async.bulk (TMA,
 //       SASS UBLKCP) completing on mbarriers.  Forward pass: in three chunks of z-planes, each issued by a warp
 //       without z rows as soon as the z sweep of the PREVIOUS group has read those planes (the load runs under the
-//       z sweep).  Backward pass: one copy per group, the next group prefetched into L2 meanwhile.
+//       z sweep).  Backward pass: six chunks; ghost planes under the y and x sweeps, interior planes after the x sweep.
 //   H1-H7 three in-place sweeps, one thread per row (rtvd_march), rows shrinking 22x22 -> 16x22 -> 16x16
-//   H9  the last sweep streams the 16^3 interior to HBM (forward: straight from the registers of the z march,
-//       64-byte segments; backward: in place, then a 128-bit coalesced copy-out)
+//   H9  the last sweep streams the 16^3 interior to HBM straight from the registers of the march (forward, z march:
+//       64-byte segments per half-warp; backward, x march: a thread owns a row, four cells per 128-bit store)
 #pragma once
 #include <cstdint>
 #include "rtvd_march.cuh"
@@ -517,15 +517,10 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             }
             sweep<1, 0, NP, NG, PS, false, false, WANT_FACE, false>(smem, gc, out_g, face_g, speed, threadIdx.x, nogate);
             __syncthreads();
-            // last sweep: along x, in place; then a coalesced 128-bit copy-out of the interior, chunk by chunk, each
-            // chunk's planes handed to the bulk copies of the next group as soon as they have been read
-#ifndef GAMER_BWD_DIRECT
-#define GAMER_BWD_DIRECT 1
-#endif
-#if GAMER_BWD_DIRECT
             // last sweep: along x, every thread sends its row to HBM itself, four cells per 128-bit store (lanes 64 B
-            // apart: half of every sector written per store, the other half by the next one); no copy-out, and all the
-            // interior planes are handed to the next group's bulk copies at once
+            // apart: half of every sector written per store, the other half by the next one), and all the interior planes
+            // are handed to the next group's bulk copies at once.  (In place + a coalesced copy-out, chunk by chunk:
+            // 115.3 against 114.7 ns/group; DESIGN.md 6 has this and the other variants.)
             sweep<0, NG, PS, NG, PS, true, true, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
                                                                         nogate);
             if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);
@@ -533,36 +528,6 @@ hydro_advance_kernel(const float* __restrict__ in, float* __restrict__ out, long
             if (threadIdx.x == 0 && has_next) {
                 fence_proxy_async();
                 for (int c = 1; c < N_BCHUNK - 1; ++c) load_bchunk(smem, ctl, in_next, c);
-            }
-            continue;
-#endif
-            sweep<0, NG, PS, NG, PS, true, false, WANT_FACE, WANT_SPEED>(smem, gc, out_g, face_g, speed, threadIdx.x,
-                                                                         nogate);
-            if (WANT_SPEED && warp < PS * PS / 32) reduce_speed(ctl, speed, it, PS * PS / 32, group_maxspeed + g);
-            __syncthreads();
-            constexpr int PER_CHUNK = NCOMP * BCHUNK_PLANES * PS * 4;       // float4 per chunk
-#pragma unroll 1
-            for (int c = 1; c < N_BCHUNK - 1; ++c) {
-                // 16 B = 4 cells of a 16-cell row; a row starts at cell 3, 4 bytes off an 8-byte boundary of shared memory:
-                // scalar, 64-bit, scalar (shifting the rows onto 16-byte boundaries costs the x march its
-                // conflict-free 64-bit stores: no gain)
-#pragma unroll
-                for (int i0 = 0; i0 < PER_CHUNK; i0 += BLOCK_THREADS) {
-                    const int i = i0 + threadIdx.x;
-                    if (i < PER_CHUNK) {
-                        const int x4 = i & 3, y = (i >> 2) & 15, zc = (i >> 6) % BCHUNK_PLANES, v = i / (64 * BCHUNK_PLANES);
-                        const int z = (c - 1) * BCHUNK_PLANES + zc;
-                        const float* sp = smem + v * VAR_FLOATS + (z + NG) * (NP * NP) + (y + NG) * NP + NG + 4 * x4;
-                        const float2 mid = *reinterpret_cast<const float2*>(sp + 1);
-                        reinterpret_cast<float4*>(out_g)[(v * PS + z) * (PS * 4) + y * 4 + x4] =
-                            make_float4(sp[0], mid.x, mid.y, sp[3]);
-                    }
-                }
-                __syncthreads();          // every thread is done with the chunk before the bulk copy overwrites it
-                if (threadIdx.x == 0 && has_next) {
-                    fence_proxy_async();
-                    load_bchunk(smem, ctl, in_next, c);
-                }
             }
         }
     }
