@@ -139,10 +139,12 @@ def test_config4_all_groups():
     check_parity(gpu_b, c["inp"][:512], c["dt"], c["dh"], c["gamma"], backward=1)
 
 
-def test_config5_full_size_sampled():
-    """32 768 groups, filled on the device (6.98 GB in, 2.68 GB out), the launch configuration bench.py times.
-    Every hot group and a sample of background groups are compared with the oracle one by one; every background
-    group must come back bit-identical to its (uniform) input."""
+@pytest.mark.parametrize("backward", [0, 1])
+def test_config5_full_size_sampled(backward):
+    """32 768 groups, filled on the device (6.98 GB in, 2.68 GB out), the launch configuration bench.py times (and the
+    same with the backward sweep order, the other half of every step of the paper).  Every hot group and a sample of
+    background groups are compared with the oracle one by one; every background group must come back bit-identical to
+    its (uniform) input."""
     torch = torch_mod()
     n = W.CONFIG5["n_groups"]
     hot = W.config5_hot_groups(n)
@@ -153,7 +155,7 @@ def test_config5_full_size_sampled():
     d_in[torch.from_numpy(hot).cuda()] = ht
     d_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32, device="cuda")
     dt, dh, gamma = W.config5_dt(), W.CONFIG5["dh"], W.CONFIG5["gamma"]
-    hydro.gamer_hydro_advance(d_in, d_out, n, 3, dt, dh, gamma)
+    hydro.gamer_hydro_advance_ex(d_in, d_out, n, 3, dt, dh, gamma, backward, None, None)
     torch.cuda.synchronize()
     is_hot = torch.zeros(n, dtype=torch.bool, device="cuda")
     is_hot[torch.from_numpy(hot).cuda()] = True
@@ -165,7 +167,7 @@ def test_config5_full_size_sampled():
     sample = np.unique(sample)
     c = W.config5(sample, n)
     gpu = d_out[torch.from_numpy(sample).cuda()].cpu().numpy()
-    check_parity(gpu, c["inp"], dt, dh, gamma)
+    check_parity(gpu, c["inp"], dt, dh, gamma, backward=backward)
     del d_in, d_out
     torch.cuda.empty_cache()
 
