@@ -11,6 +11,11 @@ sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    # The product never builds itself (hydro.lib() fails loudly without libgamer_hydro.so); the TEST SESSION may: a fresh
+    # checkout has no binaries, nvcc cross-compiles without a device, and build() is a no-op when the library is newer
+    # than its sources.
+    from paper_0907_3390_b200 import build as cuda_build
+    cuda_build.build()
 
 
 def pytest_collection_modifyitems(config, items):
