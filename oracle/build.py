@@ -16,11 +16,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if (not force) and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
         return LIB
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-Wextra", "-o", LIB + ".tmp", SRC]
+           "-Wall", "-Wextra", "-o", LIB + ".tmp%d" % os.getpid(), SRC]      # per process: concurrent builders do not collide
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
+    os.replace(LIB + ".tmp%d" % os.getpid(), LIB)
     return LIB
 
 

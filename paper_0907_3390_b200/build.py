@@ -29,11 +29,12 @@ def build(force=False, verbose=False, extra=(), out=None):
     lib = out or LIB
     if (not force) and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in DEPS):
         return lib
-    cmd = [nvcc()] + NVCC_FLAGS + list(extra) + ["-o", lib + ".tmp"] + SOURCES
+    tmp = lib + ".tmp%d" % os.getpid()          # per process: concurrent builders do not collide
+    cmd = [nvcc()] + NVCC_FLAGS + list(extra) + ["-o", tmp] + SOURCES
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
-    os.replace(lib + ".tmp", lib)
+    os.replace(tmp, lib)
     return lib
 
 

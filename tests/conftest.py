@@ -16,6 +16,8 @@ def pytest_configure(config):
     # than its sources.
     from paper_0907_3390_b200 import build as cuda_build
     cuda_build.build()
+    from oracle import build as oracle_build       # the checker too, before any test starts worker processes
+    oracle_build.build()
 
 
 def pytest_collection_modifyitems(config, items):
