@@ -128,6 +128,40 @@ GAMER_API int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx
                             int bc_x, int bc_y, int bc_z, int n_steps, int order, float cfl, float dh, float gamma,
                             float* d_work, float* d_dt_log, void* stream);
 
+/* gamer_hydro_run_uniform for callers that must not allocate device memory.
+ *
+ * WHO THIS IS FOR.  gamer_hydro_run_uniform needs 4 + gx*gy*gz floats of device scratch (d_work) and leaves it to the
+ * caller to provide them.  Some callers have nowhere to get them from once the run has started: a simulation code that
+ * hands all free device memory to its own pool at start-up, so that a later cudaMalloc simply fails; a time-step loop
+ * that other streams run beside, where an allocation would stall every one of them (cudaFree waits for all work on the
+ * device, cudaMalloc may); a plug-in that runs inside someone else's process and is told not to touch the allocator.  For them the
+ * scratch lives inside the library: a file-scope __device__ array of 4 + GAMER_NOALLOC_MAX_GROUPS floats (262 160
+ * bytes).  It is part of the library image, so EVERY GPU on which the process uses this library holds those bytes
+ * from the moment the library's code is loaded there until the process exits, whether or not this entry point is
+ * ever called.
+ *
+ * Same operation, arguments, layouts, results (bit for bit) and error conventions as gamer_hydro_run_uniform, minus
+ * d_work.  The caller still owns and passes the state (d_padded, d_interior) and the optional d_dt_log.  Differences:
+ *   - gx*gy*gz > GAMER_NOALLOC_MAX_GROUPS -> GAMER_EINVAL ("... exceeds the built-in scratch ...").  Nothing is
+ *     enqueued.  Use gamer_hydro_run_uniform with your own d_work for larger boxes.
+ *   - The call itself never calls cudaMalloc, cudaFree or any library routine that allocates; it only enqueues a
+ *     16-byte memset and kernels on `stream`.
+ *   - SET-UP: the first call on each device (with that device current) asks the runtime for the device address of the
+ *     array (cudaGetSymbolAddress; the result is kept per device) and opts the kernels into their shared-memory size.
+ *     If the library's code was not yet loaded on that device, that first call loads it.  Make this first call during
+ *     initialisation — with n_steps = 0 it changes nothing — and before any stream capture is begun.
+ *   - ONE array per device, shared by all calls: the four accumulator words are cleared at the start of every call
+ *     (stream-ordered), and the per-group speeds are written before they are read, so nothing of an earlier call leaks
+ *     into a later one that follows it in stream order.  Two calls whose work OVERLAPS on the same GPU (different
+ *     streams, or different host threads) race on the array and compute wrong time steps: serialise them, or give all
+ *     but one of them gamer_hydro_run_uniform with separate d_work. */
+#define GAMER_NOALLOC_MAX_GROUPS 65536
+GAMER_API int gamer_hydro_run_uniform_noalloc(float* d_padded, float* d_interior, int gx, int gy, int gz,
+                            int bc_x, int bc_y, int bc_z, int n_steps, int order, float cfl, float dh, float gamma,
+                            float* d_dt_log, void* stream);
+/* GAMER_NOALLOC_MAX_GROUPS as the library was built (for callers that do not compile against this header). */
+GAMER_API long long gamer_hydro_noalloc_max_groups(void);
+
 /* NEXT-4 — one pass in DOUBLE precision (the paper switches to double for its convergence tests).
  * Same operation, layouts and error conventions as gamer_hydro_advance_ex with double arrays: d_in
  * [g][v][22][22][22] (425 920 B per group), d_out [g][v][16][16][16]; backward = 0 sweeps x,y,z, 1 sweeps z,y,x;

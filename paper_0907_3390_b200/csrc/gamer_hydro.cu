@@ -238,6 +238,40 @@ march_probe_kernel(const float* __restrict__ in, gamer::GasConst gc, int k_per_s
 
 }  // namespace
 
+// Built-in scratch of gamer_hydro_run_uniform_noalloc (gamer_hydro.h): the d_work of gamer_hydro_run_uniform for callers
+// that cannot allocate.  It lives in the library image: each GPU that loads this library holds it until the process exits.
+// In HOST code the name g_noalloc_work is only a handle for the runtime (a host-side shadow), not a device address: a
+// kernel must be given what cudaGetSymbolAddress returns for the current device, never the name itself.
+static_assert(GAMER_NOALLOC_MAX_GROUPS >= 1 && GAMER_NOALLOC_MAX_GROUPS <= (1 << 20), "keep the built-in scratch modest");
+static __device__ __align__(256) float g_noalloc_work[4 + GAMER_NOALLOC_MAX_GROUPS];
+
+namespace {
+
+float* g_noalloc_ptr[64] = {};      // device address of g_noalloc_work on each device, looked up once (under g_mu)
+
+// Device address of the built-in scratch on the CURRENT device.  The first call per device does the look-up (and with
+// it loads the library's code on that device if nothing else has yet); later calls only read the cached pointer.
+int noalloc_scratch(float** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(GAMER_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e)); }
+    if (dev < 0 || dev >= 64) return fail(GAMER_ECUDA, "device ordinal %d out of range", dev);
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (g_noalloc_ptr[dev] == nullptr) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_work);
+        if (e != cudaSuccess || p == nullptr) {
+            (void)cudaGetLastError();
+            return fail(GAMER_ECUDA, "cudaGetSymbolAddress of the built-in scratch on device %d: %s", dev, cudaGetErrorString(e));
+        }
+        g_noalloc_ptr[dev] = static_cast<float*>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return GAMER_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int gamer_hydro_advance_ex(const float* d_in, float* d_out, long long n_groups, int ghost, float dt, float dh,
@@ -456,6 +490,31 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     }
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "run_uniform: %s", cudaGetErrorString(e));
     return GAMER_OK;
+}
+
+long long gamer_hydro_noalloc_max_groups(void) { return GAMER_NOALLOC_MAX_GROUPS; }
+
+// gamer_hydro_run_uniform with the library's own scratch: no cudaMalloc / cudaFree / allocating routine on this path.
+// The size is checked before the device is touched; every other argument is checked by gamer_hydro_run_uniform, which
+// also clears the accumulators (stream-ordered memset of the first 16 bytes) — the per-group speeds behind them are
+// overwritten by each step's last pass before the reduction reads them, so stale contents of an earlier call are never
+// used.
+int gamer_hydro_run_uniform_noalloc(float* d_padded, float* d_interior, int gx, int gy, int gz, int bc_x, int bc_y,
+                                    int bc_z, int n_steps, int order, float cfl, float dh, float gamma, float* d_dt_log,
+                                    void* stream) {
+    int rc = check_box(gx, gy, gz, bc_x, bc_y, bc_z);
+    if (rc != GAMER_OK) return rc;
+    const long long n = (long long)gx * gy * gz;
+    if (n > GAMER_NOALLOC_MAX_GROUPS)
+        return fail(GAMER_EINVAL,
+                    "box of %d x %d x %d = %lld groups exceeds the built-in scratch of gamer_hydro_run_uniform_noalloc "
+                    "(GAMER_NOALLOC_MAX_GROUPS = %d): call gamer_hydro_run_uniform with your own d_work",
+                    gx, gy, gz, n, GAMER_NOALLOC_MAX_GROUPS);
+    float* d_work = nullptr;
+    rc = noalloc_scratch(&d_work);
+    if (rc != GAMER_OK) return rc;
+    return gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, n_steps, order, cfl, dh, gamma,
+                                   d_work, d_dt_log, stream);
 }
 
 size_t gamer_hydro_f64_scratch_doubles(void) { return 0; }      // round 1 passed rows through device memory; tensor memory now

@@ -51,6 +51,10 @@ def lib():
         L.gamer_hydro_ghost_fill.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, vp]
         L.gamer_hydro_run_uniform.restype = ci
         L.gamer_hydro_run_uniform.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp, vp]
+        L.gamer_hydro_run_uniform_noalloc.restype = ci
+        L.gamer_hydro_run_uniform_noalloc.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp]
+        L.gamer_hydro_noalloc_max_groups.restype = ll
+        L.gamer_hydro_noalloc_max_groups.argtypes = []
         L.gamer_hydro_advance_f64.restype = ci
         L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp]
         L.gamer_hydro_advance_f64_ex.restype = ci
@@ -172,6 +176,24 @@ def gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, 
     if check:
         _check(rc)
     return rc
+
+
+def gamer_hydro_run_uniform_noalloc(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, n_steps, order, cfl, dh, gamma,
+                                    d_dt_log=None, stream=None, check=True):
+    """gamer_hydro_run_uniform without d_work, for callers that cannot allocate device memory (their pool owns it
+    all, or an allocation would stall the other streams of a running time-step loop): the scratch is a fixed array
+    inside the library, good for boxes of up to gamer_hydro_noalloc_max_groups() groups (larger ones are refused).
+    One array per GPU, shared by all calls: do not let two of them overlap on the same GPU.  Make the first call on a
+    device during start-up (n_steps = 0 does nothing else) and before any stream capture."""
+    rc = lib().gamer_hydro_run_uniform_noalloc(_ptr(d_padded), _ptr(d_interior), gx, gy, gz, bc_x, bc_y, bc_z, n_steps,
+                                               int(order), cfl, dh, gamma, _ptr(d_dt_log), _stream_ptr(stream))
+    if check:
+        _check(rc)
+    return rc
+
+
+def gamer_hydro_noalloc_max_groups():
+    return int(lib().gamer_hydro_noalloc_max_groups())
 
 
 def gamer_hydro_f64_scratch_doubles():
