@@ -390,12 +390,56 @@ def test_face_flux_of_a_perturbed_column_sits_where_the_header_says(backward):
 
 
 def test_group_max_speed_is_eq30_on_the_updated_interior():
-    """:418-426, Eq.30 — one float per group: max over the updated 16^3 cells of c_s + max_i |v_i|."""
+    """:418-426, Eq.30 — one float per group: max over the updated 16^3 cells of c_s + max_i |v_i|.  A second check on a
+    non-trivial state against workloads' own typing of Eq.30; the PIN is test_eq30_speed_worked_by_hand below."""
     c = W.config1()
     inp = c["inp"].astype(np.float64)
     out, ms = oracle.hydro_advance(inp, c["dt"], c["dh"], c["gamma"], want_maxspeed=True)
     for g in range(out.shape[0]):
         assert ms[g] == pytest.approx(W.max_signal_speed(out[g], c["gamma"]), rel=1e-14)
+
+
+def _filled_group(u5, dtype):
+    g = np.empty((1, 5, 22, 22, 22), dtype)
+    g[0] = np.asarray(u5, dtype).reshape(5, 1, 1, 1)
+    return g
+
+
+@pytest.mark.parametrize("dtype,rel", [(np.float64, 1e-15), (np.float32, 2e-7)])
+def test_eq30_speed_worked_by_hand(dtype, rel):
+    """Eq.30 (:420) pinned by values worked on paper, not by a second typing of the formula.
+    Uniform state rho = 2, v = (3, -4, 1), P = 4, gamma = 2:  c_s = sqrt(gamma P / rho) = sqrt(2*4/2) = 2,
+    max_i |v_i| = 4  ->  speed 6.  Conserved: m = (6, -8, 2), e = P/(gamma-1) + rho |v|^2 / 2 = 4 + 26 = 30.
+    Plausible mistakes and what they would give: full |v| = sqrt 26 instead of the largest component -> 7.10;
+    sum of the components -> 10; the first component only -> 5; c_s from e instead of P -> sqrt(2*30/2) + 4 = 9.48;
+    gamma - 1 instead of gamma under the root -> 5.41; max(c_s, |v|) -> 4."""
+    A = [2.0, 6.0, -8.0, 2.0, 30.0]
+    u = _filled_group(A, dtype)
+    assert oracle.max_signal_speed(u, 2.0) == pytest.approx(6.0, rel=rel)
+    # a uniform state is returned unchanged by a pass (P-uniform), so the per-group speed of the UPDATED interior is 6
+    out, ms = oracle.hydro_advance(u, 0.01, 1.0, 2.0, want_maxspeed=True)
+    assert np.array_equal(out, u[:, :, 3:19, 3:19, 3:19])
+    assert ms.shape == (1,) and ms[0] == pytest.approx(6.0, rel=rel)
+    # Non-uniform: one hand-set cell holds the maximum.  rho = 1, v = (0, 0, -7), P = 4.5, gamma = 2:
+    # c_s = sqrt(2*4.5/1) = 3, speed 10; e = 4.5 + 49/2 = 29.  dt = 0 makes the pass the identity on the interior
+    # (u' = u - 0 * flux), so the speeds of the updated cells are those of the input cells.
+    B = [1.0, 0.0, 0.0, -7.0, 29.0]
+    two = np.concatenate([u, u])
+    two[1, :, 3 + 5, 3 + 9, 3 + 12] = B                       # interior cell (k, j, i) = (5, 9, 12) of group 1
+    assert oracle.max_signal_speed(two, 2.0) == pytest.approx(10.0, rel=rel)
+    out, ms = oracle.hydro_advance(two, 0.0, 1.0, 2.0, want_maxspeed=True)
+    assert np.array_equal(out, two[:, :, 3:19, 3:19, 3:19])
+    assert ms[0] == pytest.approx(6.0, rel=rel) and ms[1] == pytest.approx(10.0, rel=rel)
+    # The same cell in a GHOST zone: the time step of reading R10 runs over all padded cells and sees it (10); the
+    # per-group value of :426 runs over the 16^3 updated cells and does not (6).
+    ghost = np.concatenate([u, u])
+    ghost[1, :, 1, 12, 15] = B                                # padded z = 1: a ghost cell
+    assert oracle.max_signal_speed(ghost, 2.0) == pytest.approx(10.0, rel=rel)
+    _, ms = oracle.hydro_advance(ghost, 0.0, 1.0, 2.0, want_maxspeed=True)
+    assert ms[1] == pytest.approx(6.0, rel=rel)
+    # and the multi-step loop turns it into dt = C dh / speed: 0.5 * 0.25 / 6
+    _, dts = oracle.run_uniform(u, (1, 1, 1), (0, 0, 0), 1, 0.5, 0.25, 2.0)
+    assert float(dts[0]) == pytest.approx(0.5 * 0.25 / 6.0, rel=max(rel, 1e-15) * 2)
 
 
 # ------------------------------------------------------------------------------------------------ precision
