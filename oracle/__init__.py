@@ -35,6 +35,9 @@ def lib():
             getattr(L, "oracle_hydro_advance_" + sfx).restype = ctypes.c_longlong
             getattr(L, "oracle_hydro_advance_" + sfx).argtypes = [p, p, ctypes.c_longlong, ctypes.c_int, ct, ct, ct,
                                                                  ctypes.c_int, ctypes.c_int, p, p, ctypes.c_int]
+            getattr(L, "oracle_hydro_advance_badmask_" + sfx).restype = ctypes.c_longlong
+            getattr(L, "oracle_hydro_advance_badmask_" + sfx).argtypes = [p, p, ctypes.c_longlong, ctypes.c_int, ct, ct, ct,
+                                                                         ctypes.c_int, ctypes.c_int, p, ctypes.c_int]
         L.oracle_count_ops.restype = None
         L.oracle_count_ops.argtypes = [ctypes.c_void_p]
         L.oracle_has_openmp.restype = ctypes.c_int
@@ -121,6 +124,25 @@ def hydro_advance(inp, dt, dh, gamma, backward=0, dtype=None, ghost=NGHOST, c_mo
     if return_bad:
         res += (bad,)
     return res if len(res) > 1 else out
+
+
+def hydro_advance_badmask(inp, dt, dh, gamma, backward=0, dtype=None, c_mode=0, n_threads=1):
+    """hydro_advance that also says WHERE the pass left the physical domain (reading R7/R17b).  Returns
+    (out [G][5][16][16][16], badmask [G][22][22][22] uint8, count): bit 0 of badmask = the cell held five finite values
+    with rho <= 0 or P <= 0 when some sweep read it; bit 1 = it held a non-finite value (what spreads from bit-0 cells,
+    at most 3 cells along the axis of each later sweep).  Bookkeeping only: `out` is hydro_advance's."""
+    dtp = np.dtype(dtype if dtype is not None else inp.dtype)
+    a = np.ascontiguousarray(inp, dtype=dtp)
+    assert a.ndim == 5 and a.shape[1:] == (NCOMP, NP, NP, NP), a.shape
+    G = a.shape[0]
+    out = np.empty((G, NCOMP, PS, PS, PS), dtp)
+    mask = np.zeros((G, NP, NP, NP), np.uint8)
+    bad = getattr(lib(), "oracle_hydro_advance_badmask_" + _sfx(dtp))(
+        a.ctypes.data, out.ctypes.data, G, NGHOST, dtp.type(dt), dtp.type(dh), dtp.type(gamma), int(backward), c_mode,
+        mask.ctypes.data, int(n_threads))
+    if bad < 0:
+        raise ValueError("oracle_hydro_advance_badmask: error %d" % bad)
+    return out, mask, int(bad)
 
 
 def count_ops():

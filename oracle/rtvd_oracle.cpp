@@ -196,9 +196,14 @@ void row_update(const T* u, T* unew, int N, T k, T gamma, int c_mode, int limite
 //                          transverse interior indices, slower first: d=x:(k,j)  d=y:(k,i)  d=z:(j,i).
 //   maxspeed               optional: max over the 16^3 updated cells of c_s + max(|v_x|,|v_y|,|v_z|), Eq.30 (:420-426)
 //   returns the number of cells (over all sweeps, on cells that are read) with rho <= 0 or P <= 0  (reading R7)
+//   badmask [22][22][22]   optional bookkeeping beside that counter (no arithmetic depends on it): WHERE such cells
+//                          were met.  bit 0: the cell held five finite values with rho <= 0 or P <= 0 when a sweep read
+//                          it (where the pass leaves the physical domain); bit 1: it held a non-finite value (what
+//                          spreads from such a cell: at most 3 cells along the axis of each later sweep, :178).
 // ------------------------------------------------------------------------------------------------
 template <typename T>
-long long advance_group(const T* in, T* out, T k, T gamma, int backward, int c_mode, T* face, T* maxspeed) {
+long long advance_group(const T* in, T* out, T k, T gamma, int backward, int c_mode, T* face, T* maxspeed,
+                        unsigned char* badmask = nullptr) {
     const size_t NV = (size_t)NP * NP * NP;
     std::vector<T> W(in, in + NCOMP * NV);
     auto idx = [](int v, int z, int y, int x) { return (((size_t)v * NP + z) * NP + y) * NP + x; };
@@ -226,7 +231,17 @@ long long advance_group(const T* in, T* out, T k, T gamma, int backward, int c_m
                     const T ek = (row[1 * NP + n] * row[1 * NP + n] +
                                   (row[2 * NP + n] * row[2 * NP + n] + row[3 * NP + n] * row[3 * NP + n])) / (T(2) * rho);
                     const T P = (gamma - T(1)) * (row[4 * NP + n] - ek);
-                    if (!(rho > T(0)) || !(P > T(0))) ++bad;
+                    if (!(rho > T(0)) || !(P > T(0))) {
+                        ++bad;
+                        if (badmask) {
+                            bool finite = true;
+                            for (int q = 0; q < NCOMP; ++q) {
+                                const double val = to_double(row[q * NP + n]);
+                                finite = finite && (val - val == 0.0);       // false for NaN and +-Inf
+                            }
+                            badmask[((size_t)a[2] * NP + a[1]) * NP + a[0]] |= finite ? 1 : 2;
+                        }
+                    }
                 }
                 row_update<T>(row, rnew, NP, k, gamma, c_mode, 1, nullptr, face ? fh : nullptr);
                 for (int n = NGHOST; n < NP - NGHOST; ++n) {
@@ -276,7 +291,7 @@ long long advance_group(const T* in, T* out, T k, T gamma, int backward, int c_m
 
 template <typename T>
 long long advance_batch(const T* in, T* out, long long n_groups, int ghost, T dt, T dh, T gamma, int backward,
-                        int c_mode, T* face, T* maxspeed, int n_threads) {
+                        int c_mode, T* face, T* maxspeed, int n_threads, unsigned char* badmask = nullptr) {
     if (ghost != NGHOST) return -2;
     if (n_groups < 0) return -1;
     const T k = dt / dh;
@@ -289,7 +304,8 @@ long long advance_batch(const T* in, T* out, long long n_groups, int ghost, T dt
 #endif
     for (long long g = 0; g < n_groups; ++g)
         bad += advance_group<T>(in + g * in_stride, out + g * out_stride, k, gamma, backward, c_mode,
-                                face ? face + g * face_stride : nullptr, maxspeed ? maxspeed + g : nullptr);
+                                face ? face + g * face_stride : nullptr, maxspeed ? maxspeed + g : nullptr,
+                                badmask ? badmask + g * (size_t)NP * NP * NP : nullptr);
     return bad;
 }
 
@@ -339,6 +355,20 @@ long long oracle_hydro_advance_f64(const double* in, double* out, long long n_gr
                                    int n_threads) {
     return advance_batch<double>(in, out, n_groups, ghost, dt, dh, gamma, backward, c_mode, face_flux, maxspeed,
                                  n_threads);
+}
+
+// The same pass; additionally badmask[g][22][22][22] (zeroed by the caller) receives where non-physical cells were met
+// (bits as described at advance_group).  Bookkeeping only: the results are those of oracle_hydro_advance_*.
+long long oracle_hydro_advance_badmask_f32(const float* in, float* out, long long n_groups, int ghost, float dt, float dh,
+                                           float gamma, int backward, int c_mode, unsigned char* badmask, int n_threads) {
+    return advance_batch<float>(in, out, n_groups, ghost, dt, dh, gamma, backward, c_mode, nullptr, nullptr, n_threads,
+                                badmask);
+}
+long long oracle_hydro_advance_badmask_f64(const double* in, double* out, long long n_groups, int ghost, double dt,
+                                           double dh, double gamma, int backward, int c_mode, unsigned char* badmask,
+                                           int n_threads) {
+    return advance_batch<double>(in, out, n_groups, ghost, dt, dh, gamma, backward, c_mode, nullptr, nullptr, n_threads,
+                                 badmask);
 }
 
 // Measured operation count of one patch-group pass (replaces the hand count of SURVEY.md 8(d)).

@@ -28,3 +28,28 @@ def physical_mask(inp, dt, dh, gamma, backward=0, n_threads=8):
     bad64 = np.array([r[1] for r in r64])
     finite = np.isfinite(out32).all(axis=(1, 2, 3, 4)) & np.isfinite(out64).all(axis=(1, 2, 3, 4))
     return (bad32 == 0) & (bad64 == 0) & finite, out32, out64, bad32, bad64
+
+
+def dilate3(mask):
+    """mask [G][22][22][22] bool -> the same with every set cell grown by 3 cells along each axis (a 7^3 box, clipped at
+    the edge of the padded group).  This is the domain of dependence of one pass (a sweep reaches 3 cells
+    along its own axis, and the three sweeps of a pass act along x, y and z in turn): a cell that was non-physical when
+    some sweep read it can change the pass's result at most inside this box, and nothing outside it."""
+    d = np.asarray(mask, bool)
+    for ax in (1, 2, 3):
+        n = d.shape[ax]
+        acc = d.copy()
+        for sh in (1, 2, 3):
+            to, fr = [slice(None)] * 4, [slice(None)] * 4
+            to[ax], fr[ax] = slice(sh, n), slice(0, n - sh)
+            acc[tuple(to)] |= d[tuple(fr)]
+            to[ax], fr[ax] = slice(0, n - sh), slice(sh, n)
+            acc[tuple(to)] |= d[tuple(fr)]
+        d = acc
+    return d
+
+
+def outside(keep, a, dummy):
+    """a [G][5][16][16][16] with the cells where keep [G][16][16][16] is False replaced by the physical state `dummy`
+    (5 values), so that a whole-array comparison runs over the kept cells only."""
+    return np.where(keep[:, None], a, np.asarray(dummy, a.dtype).reshape(1, 5, 1, 1, 1))

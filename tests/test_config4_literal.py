@@ -1,30 +1,39 @@
 """Config 4 exactly as BASELINE.json configs[3] and SURVEY.md 8(c)#17 word it: ln rho Gaussian with 3-D power ~ k^-3,
-sigma(ln rho) = 2.  (workloads.config4, the k^-5 field of DESIGN.md reading R17, stays the all-groups config-4 case.)
+sigma(ln rho) = 2.  (workloads.config4, the k^-5 field of DESIGN.md reading R17, stays the timed config-4 case.)
 
 The scheme has no floor (the paper names none; R7) and neither side adds one: on this field 2243 of the 4096
 groups meet a cell with rho <= 0 or P <= 0 somewhere along the pass, on the CPU oracle in fp32 and in fp64 alike
-(17 967 such cells each).  Parity is checked on the 1853 groups that stay physical on both; on the others the
-CUDA path is only required to agree with the oracle on WHERE the result is finite (same arithmetic, same breakdown)."""
+(17 967 reads of such cells each; 5474 distinct cells where the state was still finite, the rest is what spreads from
+them).  The oracle reports WHERE (oracle.hydro_advance_badmask); a non-physical cell can only change results within 3
+cells along each axis (the domain of dependence of one pass), so the CUDA path is compared with the fp32
+and the fp64 oracle on EVERY interior cell outside that 7^3 neighbourhood, on all 4096 groups: 95.1 % of the config's
+interior cells (stated in BASELINE.md).  Inside it both sides compute NaN/Inf or meaningless numbers and nothing is
+claimed."""
 import functools
 
 import numpy as np
 import pytest
 
+import oracle
 import physical_groups as PG
 from paper_0907_3390_b200 import workloads as W
 
-N_PHYSICAL = 1853          # of 4096; stated in BASELINE.md
+N_PHYSICAL = 1853          # groups that meet no non-physical cell at all, of 4096; stated in BASELINE.md
+DUMMY = (1.0, 0.0, 0.0, 0.0, 1.0)
 
 
 @functools.lru_cache(maxsize=1)
 def literal():
     c = W.config4_literal()
-    mask, o32, o64, bad32, bad64 = PG.physical_mask(c["inp"], c["dt"], c["dh"], c["gamma"])
-    return c, mask, o32, o64, bad32, bad64
+    o32, m32, bad32 = oracle.hydro_advance_badmask(c["inp"], c["dt"], c["dh"], c["gamma"], n_threads=16)
+    o64, m64, bad64 = oracle.hydro_advance_badmask(c["inp"], c["dt"], c["dh"], c["gamma"], dtype=np.float64, n_threads=16)
+    left = ((m32 | m64) & 1).astype(bool)                    # where the pass left the physical domain, either precision
+    keep = ~PG.dilate3(left)[:, 3:19, 3:19, 3:19]            # interior cells that no such cell can have touched
+    return c, o32, o64, m32, m64, (bad32, bad64), keep
 
 
 def test_literal_field_is_the_stated_recipe_and_most_of_it_leaves_the_physical_domain():
-    c, mask, o32, o64, bad32, bad64 = literal()
+    c, o32, o64, m32, m64, (bad32, bad64), keep = literal()
     inp = c["inp"]
     assert inp.shape == (4096, 5, 22, 22, 22) and inp.dtype == np.float32
     lnrho = np.log(inp[:, 0, 3:19, 3:19, 3:19].astype(np.float64))
@@ -38,19 +47,46 @@ def test_literal_field_is_the_stated_recipe_and_most_of_it_leaves_the_physical_d
     assert -3.3 <= np.log2(hi / lo) / 2.0 <= -2.7
     # every input cell is physical; it is the pass that leaves the physical domain
     assert (inp[:, 0] > 0).all()
-    assert int(mask.sum()) == N_PHYSICAL
-    assert int((bad32 > 0).sum()) == int((bad64 > 0).sum()) == 2243
-    assert int(bad32.sum()) == int(bad64.sum())                                 # the same cells in both precisions
-    # P-fp on the groups that stay physical (metric R11)
-    e = W.parity_error(o32[mask], o64[mask], c["gamma"])
+    hit32, hit64 = m32.any(axis=(1, 2, 3)), m64.any(axis=(1, 2, 3))
+    fin = np.isfinite(o32).all(axis=(1, 2, 3, 4)) & np.isfinite(o64).all(axis=(1, 2, 3, 4))
+    assert int((~hit32 & ~hit64 & fin).sum()) == N_PHYSICAL
+    assert int(hit32.sum()) == int(hit64.sum()) == 2243
+    assert bad32 == bad64 == 17967                                              # the same reads in both precisions
+    assert np.array_equal(m32, m64)                                             # ... of the same cells
+    assert int((m32 & 1).astype(bool).sum()) == 5474
+    # the bookkeeping variant returns hydro_advance's results
+    ref = oracle.hydro_advance(inp[:32], c["dt"], c["dh"], c["gamma"], return_bad=True)[0]
+    assert np.array_equal(ref, o32[:32], equal_nan=True)
+
+
+def test_dilation_is_the_7_cubed_box_clipped_at_the_edges():
+    m = np.zeros((1, 22, 22, 22), bool)
+    m[0, 10, 11, 12] = m[0, 0, 21, 5] = True
+    d = PG.dilate3(m)
+    want = np.zeros_like(m)
+    want[0, 7:14, 8:15, 9:16] = True
+    want[0, 0:4, 18:22, 2:9] = True
+    assert np.array_equal(d, want)
+
+
+def test_nothing_non_finite_outside_the_domain_of_dependence_and_fp32_tracks_fp64_there():
+    """What the mask is for: outside the 3-cell neighbourhood of the cells where the pass left the physical domain the
+    oracle's result is finite and well conditioned (fp32 against fp64 at the P-fp bar, metric R11) on every group."""
+    c, o32, o64, _, _, _, keep = literal()
+    frac = keep.mean()
+    print("literal config 4: %.2f %% of the interior cells lie outside the domain of dependence" % (100 * frac))
+    assert frac > 0.95, frac
+    assert np.isfinite(o32[np.broadcast_to(keep[:, None], o32.shape)]).all()
+    assert np.isfinite(o64[np.broadcast_to(keep[:, None], o64.shape)]).all()
+    e = W.parity_error(PG.outside(keep, o32, DUMMY), PG.outside(keep, o64, DUMMY), c["gamma"])
     assert e["max_rel"] <= 1e-4, e
 
 
 @pytest.mark.gpu
-def test_gpu_parity_on_the_physical_groups_of_the_literal_config4():
+def test_gpu_parity_on_every_group_of_the_literal_config4_outside_the_domain_of_dependence():
     import torch
     from paper_0907_3390_b200 import hydro
-    c, mask, o32, o64, _, _ = literal()
+    c, o32, o64, _, _, _, keep = literal()
     inp = c["inp"]
     G = inp.shape[0]
     d_in = torch.from_numpy(inp).cuda()
@@ -58,14 +94,12 @@ def test_gpu_parity_on_the_physical_groups_of_the_literal_config4():
     hydro.gamer_hydro_advance(d_in, d_out, G, 3, c["dt"], c["dh"], c["gamma"])
     torch.cuda.synchronize()
     gpu = d_out.cpu().numpy()
-    e32 = W.parity_error(gpu[mask], o32[mask], c["gamma"])
-    e64 = W.parity_error(gpu[mask], o64[mask], c["gamma"])
-    print("literal config 4: %d of %d groups physical; GPU vs fp32 oracle %.3g, vs fp64 oracle %.3g"
-          % (mask.sum(), G, e32["max_rel"], e64["max_rel"]))
+    # exact agreement on finiteness outside the mask: the oracle is finite there (CPU test above), so is the CUDA path
+    assert np.isfinite(gpu[np.broadcast_to(keep[:, None], gpu.shape)]).all()
+    g = PG.outside(keep, gpu, DUMMY)
+    e32 = W.parity_error(g, PG.outside(keep, o32, DUMMY), c["gamma"])
+    e64 = W.parity_error(g, PG.outside(keep, o64, DUMMY), c["gamma"])
+    print("literal config 4: all %d groups, %.2f %% of the interior cells compared; GPU vs fp32 oracle %.3g, vs fp64 "
+          "oracle %.3g" % (G, 100 * keep.mean(), e32["max_rel"], e64["max_rel"]))
     assert e32["max_rel"] <= 1e-5, e32
     assert e64["max_rel"] <= 1e-4, e64
-    # groups whose oracle result is finite everywhere are finite on the GPU too (no floor on either side)
-    fin_o = np.isfinite(o32).all(axis=(1, 2, 3, 4))
-    fin_g = np.isfinite(gpu).all(axis=(1, 2, 3, 4))
-    assert (fin_g[mask]).all()
-    assert (fin_o == fin_g).mean() > 0.99
