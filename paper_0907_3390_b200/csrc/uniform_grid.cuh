@@ -14,6 +14,7 @@ namespace gamer {
 struct BoxGeom {
     int gx, gy, gz;          // groups along x, y, z; group index g = (kz * gy + ky) * gx + kx
     int bc[3];               // per axis x, y, z: 0 = periodic, 1 = leave the ghost cells beyond the box untouched
+    int nseg;                // ghost fill only: segments the walk along x is cut into (ghost_fill_segments)
 };
 
 // One CTA per (strip of groups along x, variable): the CTA walks kx = 0 .. gx-1 and assembles the 22^3 padded cells of
@@ -27,12 +28,23 @@ struct BoxGeom {
 //     of the x neighbours exists (the first version spent a quarter of its time on those 12-byte reads).  The walk
 //     therefore runs from kx = -1 (wrap: only remembered) to kx = gx (wrap: only its first quarters are used), and two
 //     tiles are in flight: tile kx is being filled while tile kx-1 receives its last ghost cells and leaves.
+//   * A thin box (few strips: a Sod column has gy = gz = 1, so 5 CTAs) would leave most SMs idle: the walk is then cut
+//     into nseg segments [x0, x1) of the strip, one CTA each, until there are about two CTAs per SM.  A segment starts
+//     one group early and ends one group late like the whole walk does, at the cost of one extra quarter-row load at
+//     each segment end.
 constexpr int GF_THREADS = 256;
 constexpr int GF_ROWS = NP * NP;                                  // 484 padded (z,y) rows
 constexpr int GF_ITEMS = (GF_ROWS * 4 + GF_THREADS - 1) / GF_THREADS;   // 8 quarter rows per thread (the last one partial)
 constexpr int GF_SMEM_BYTES = 2 * VAR_FLOATS * 4 + 2 * NP * 8;    // two tiles + the y and z offset tables
-// number of CTAs that ghost_fill_kernel needs for a box of gx x gy x gz groups
-inline long long ghost_fill_ctas(int gx, int gy, int gz) { (void)gx; return (long long)gy * gz * NCOMP; }
+// segments per strip: 1 when the strips alone give two CTAs per SM, else as many as that takes (at most gx)
+inline int ghost_fill_segments(int gx, int gy, int gz, int sm_count) {
+    const long long strips = (long long)gy * gz * NCOMP, want = 2ll * sm_count;
+    if (strips >= want) return 1;
+    const long long nseg = (want + strips - 1) / strips;
+    return (int)(nseg < gx ? nseg : gx);
+}
+// number of CTAs that ghost_fill_kernel needs for a box of gx x gy x gz groups cut into nseg segments along x
+inline long long ghost_fill_ctas(int gx, int gy, int gz, int nseg = 1) { (void)gx; return (long long)gy * gz * NCOMP * nseg; }
 
 __global__ void __launch_bounds__(GF_THREADS, 2)
 ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded, BoxGeom geo) {
@@ -41,8 +53,10 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
     long long* const off_y = reinterpret_cast<long long*>(gf_smem + 2 * VAR_FLOATS * 4);
     long long* const off_z = off_y + NP;
     const int v = blockIdx.x % NCOMP;
-    const int strip = blockIdx.x / NCOMP;
+    const int strips = geo.gy * geo.gz;
+    const int strip = (blockIdx.x / NCOMP) % strips, seg = blockIdx.x / (NCOMP * strips);
     const int ky = strip % geo.gy, kz = strip / geo.gy;
+    const int x0 = (int)((long long)seg * geo.gx / geo.nseg), x1 = (int)((long long)(seg + 1) * geo.gx / geo.nseg);
     // Per padded y and z: offset (in floats) of the source row inside `interior`, or -1 = beyond a "keep" end.
     constexpr long long GS = (long long)NCOMP * PS * PS * PS;     // floats per group of `interior`
     if (threadIdx.x < 2 * NP) {
@@ -73,21 +87,21 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
     }
     const long long g0 = ((long long)kz * geo.gy + ky) * geo.gx;  // group index of kx = 0 in this strip
     float4 prev[GF_ITEMS];                                         // the quarters loaded one step earlier (group kx-1)
-    for (int kx = -1; kx <= geo.gx; ++kx) {
+    for (int kx = x0 - 1; kx <= x1; ++kx) {
         const int ks = kx < 0 ? geo.gx - 1 : (kx == geo.gx ? 0 : kx);          // group whose interior is read (wrap)
-        const bool fill = kx >= 0 && kx < geo.gx;                                // tile kx exists
+        const bool fill = kx >= x0 && kx < x1;                                   // tile kx exists (in this segment)
         const bool wrap_l = kx == 0 && geo.bc[0], wrap_r = kx == geo.gx && geo.bc[0];   // "keep" ends along x
         float* const tile = tiles + (kx & 1) * VAR_FLOATS;                      // tile of group kx
         float* const tprev = tiles + ((kx + 1) & 1) * VAR_FLOATS;               // tile of group kx-1
-        float* const dst = padded + ((g0 + (fill ? kx : 0)) * NCOMP + v) * (long long)VAR_FLOATS;
-        float* const dprev = padded + ((g0 + (kx > 0 ? kx - 1 : 0)) * NCOMP + v) * (long long)VAR_FLOATS;
+        float* const dst = padded + ((g0 + (fill ? kx : x0)) * NCOMP + v) * (long long)VAR_FLOATS;
+        float* const dprev = padded + ((g0 + (kx > x0 ? kx - 1 : x0)) * NCOMP + v) * (long long)VAR_FLOATS;
         // the bulk store that last read `tile` (group kx-2) must have finished reading before anybody writes to it
         if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         __syncthreads();
         const float* const src = src_v + ks * GS;
         float4 q[GF_ITEMS];
         // only the quarters that are used are loaded: all of them for a tile, the first / last ones at the two wraps
-        const bool need = fill || (kx < 0 && part == 3) || (kx == geo.gx && part == 0);
+        const bool need = fill || (kx < x0 && part == 3) || (kx == x1 && part == 0);
 #pragma unroll
         for (int k = 0; k < GF_ITEMS; ++k) {
             const int row = (threadIdx.x >> 2) + (GF_THREADS / 4) * k;
@@ -116,7 +130,7 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
                         }
                     }
                 }
-                if (kx > 0 && part == 0) {                         // ghost cells x = 19..21 of group kx-1: cells 0..2 here
+                if (kx > x0 && part == 0) {                        // ghost cells x = 19..21 of group kx-1: cells 0..2 here
                     float* r = tprev + row * NP + NG + PS;
                     if (keep_row || wrap_r) {
                         const float* e = dprev + row * NP + NG + PS;
@@ -131,7 +145,7 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
         // tile kx-1 is complete: make the generic-proxy writes visible to the async proxy and let it go
         fence_proxy_async();
         __syncthreads();
-        if (threadIdx.x == 0 && kx > 0) {
+        if (threadIdx.x == 0 && kx > x0) {
             asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dprev), "r"(smem_u32(tprev)),
                          "r"(VAR_FLOATS * 4)
                          : "memory");

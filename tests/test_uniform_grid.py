@@ -155,7 +155,11 @@ def test_ghost_fill_argument_validation_needs_no_device():
 # ---------------------------------------------------------------------------------------------------------- GPU
 @pytest.mark.gpu
 @pytest.mark.parametrize("grid,bc", [((1, 1, 1), (0, 0, 0)), ((2, 3, 2), (0, 0, 0)), ((2, 2, 3), (1, 0, 0)),
-                                     ((3, 2, 2), (0, 1, 1)), ((2, 2, 2), (1, 1, 1))])
+                                     ((3, 2, 2), (0, 1, 1)), ((2, 2, 2), (1, 1, 1)),
+                                     # thin boxes: the walk along x is cut into segments (one group each for gx = 8,
+                                     # one or two groups each for gx = 70 with 5 strips on 148 SMs)
+                                     ((1, 1, 8), (0, 0, 0)), ((1, 1, 8), (1, 0, 0)), ((1, 1, 70), (0, 0, 0)),
+                                     ((1, 1, 70), (1, 0, 0)), ((1, 2, 45), (0, 1, 0))])
 def test_gpu_ghost_fill_bit_exact(grid, bc):
     import torch
     gz, gy, gx = grid
