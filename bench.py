@@ -248,7 +248,7 @@ def run_reference(args):
 
 def run_ours(args):
     import torch
-    from paper_0907_3390_b200 import hydro
+    from paper_0907_3390_b200 import hydro, probes
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -330,7 +330,7 @@ def run_ours(args):
                                                   "uses this one, the measured FMA rate is beside it" % n_sm)
     # the FMA-only micro-benchmark of the library, measured in this run
     d_sink = torch.zeros(4, dtype=torch.float32, device=device)
-    peak_meas_tf, peak_meas_lanes = hydro.gamer_hydro_fp32_peak(5, d_sink, peaks["sm_max_mhz"])
+    peak_meas_tf, peak_meas_lanes = probes.gamer_probe_fp32_peak(5, d_sink, peaks["sm_max_mhz"])
     roofline_alu["peak_measured_tflops"] = peak_meas_tf
     roofline_alu["peak_measured_fma_per_clk_per_sm"] = peak_meas_lanes
     roofline_alu["frac_of_measured_peak"] = ach_tf / peak_meas_tf
@@ -338,14 +338,14 @@ def run_ours(args):
     # slot with 1..4 warps per sub-partition, no loads, no barriers; and the cost of an FMA with three distinct registers
     issue_probe = None
     if rank == 0:
-        ffma3 = hydro.gamer_hydro_issue_probe(0, 4)
-        march = {ax: [hydro.gamer_hydro_issue_probe(i + 1, k) for k in (1, 2, 3, 4)] for i, ax in enumerate("xyz")}
+        ffma3 = probes.gamer_probe_issue(0, 4)
+        march = {ax: [probes.gamer_probe_issue(i + 1, k) for k in (1, 2, 3, 4)] for i, ax in enumerate("xyz")}
         # a group is 16 x-, 11 y-, 8 z-marches on 4 sub-partitions: with every slot filled at the 4-warp rate
         packed = (16 * march["x"][3] + 11 * march["y"][3] + 8 * march["z"][3]) / 4.0
         # the kernel's three phases run 4, 3 and 2 warps per sub-partition
         phases = 4 * march["x"][3] + 3 * march["y"][2] + 2 * march["z"][1]
         clk = peaks["sm_max_mhz"] * 1e6
-        issue_probe = dict(api="gamer_hydro_issue_probe", ffma_3_distinct_registers_clocks_per_instr=ffma3,
+        issue_probe = dict(api="gamer_probe_issue (libgamer_probes.so)", ffma_3_distinct_registers_clocks_per_instr=ffma3,
                            clocks_per_warp_march_by_warps_per_subpartition=march,
                            ns_per_group_if_every_slot_ran_at_the_4_warp_rate=packed / clk * 1e9 / n_sm,
                            ns_per_group_sum_of_the_three_phases=phases / clk * 1e9 / n_sm)
@@ -430,6 +430,48 @@ def run_ours(args):
                        h2d_bytes_per_step=int(h_in.numel() * 4), d2h_bytes_per_step=int(h_out.numel() * 4),
                        steps=e2e_steps, ms_per_step=1e3 * wall / e2e_steps, groups_per_chunk=chunk, n_streams=ns,
                        h2d_gbs=h_in.numel() * 4 * e2e_steps / wall / 1e9, api="gamer_hydro_pipeline_run (pinned host)")
+            e2e["d2h_gbs"] = h_out.numel() * 4 * e2e_steps / wall / 1e9
+            # The pipeline's own report (SURVEY.md 8(d) "Pipeline subsystem"; PAPER.md:354-356 Fig.5, :368): the link
+            # measured in the same run on the same pinned buffers, then one pass per (N_g, N_s) point.
+            if world == 1 and not args.no_pipeline_sweep:
+                def copy_ms(pairs):
+                    """[(dst, src, stream)] started together; returns ms until the last one is done (device events)."""
+                    torch.cuda.synchronize()
+                    ev = []
+                    for dst, src, st in pairs:
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        with torch.cuda.stream(st):
+                            e0.record(st)
+                            dst.copy_(src, non_blocking=True)
+                            e1.record(st)
+                        ev.append((e0, e1))
+                    torch.cuda.synchronize()
+                    return max(ev[0][0].elapsed_time(e1) for _, e1 in ev)
+                s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+                in_b, out_b = h_in.numel() * 4, h_out.numel() * 4
+                copy_ms([(d_in, h_in, s1)])                                            # warm-up (h_in holds d_in's data)
+                t_h2d = min(copy_ms([(d_in, h_in, s1)]) for _ in range(2))
+                t_d2h = min(copy_ms([(h_out, d_out, s2)]) for _ in range(2))
+                t_both = min(copy_ms([(d_in, h_in, s1), (h_out, d_out, s2)]) for _ in range(2))
+                link = dict(h2d_alone_gbs=in_b / t_h2d / 1e6, d2h_alone_gbs=out_b / t_d2h / 1e6,
+                            both_at_once_ms=t_both, both_at_once_h2d_gbs=in_b / t_both / 1e6,
+                            both_at_once_d2h_gbs=out_b / t_both / 1e6, api="pinned cudaMemcpyAsync (torch copy_)")
+                points = [(chunk, 1), (chunk, 2), (chunk, 4), (1024, 4), (2048, 4), (4096, 4)]
+                sweep = []
+                for ng, nst in points:
+                    ng = min(ng, n)
+                    hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, dt, dh, gamma, 0, ng, nst)      # staging grows here
+                    t0 = time.perf_counter()
+                    hydro.gamer_hydro_pipeline_run(h_in, h_out, n, 3, dt, dh, gamma, 0, ng, nst)
+                    w = (time.perf_counter() - t0) * 1e3
+                    # what a perfect overlap leaves: the longest of the three serial sums (copies at the alone rates)
+                    sweep.append(dict(groups_per_chunk=ng, n_streams=nst, wall_ms=w, h2d_gbs=in_b / w / 1e6,
+                                      d2h_gbs=out_b / w / 1e6, sum_h2d_ms=t_h2d, sum_kernel_ms=kernel_ms, sum_d2h_ms=t_d2h,
+                                      overlap_efficiency=max(t_h2d, kernel_ms, t_d2h) / w,
+                                      serial_ms=t_h2d + kernel_ms + t_d2h))
+                e2e["pipeline"] = dict(link=link, sweep=sweep,
+                                       note="overlap_efficiency = max(sum H2D, sum kernel, sum D2H) / wall; the sums are "
+                                            "the whole batch at the alone-measured rates and the device-timed kernel")
             del h_in, h_out
             hydro.gamer_hydro_pipeline_release()
         except Exception as ex:      # e.g. not enough pinnable host memory
@@ -460,20 +502,19 @@ def run_ours(args):
         n64 = min(n, 8192)
         d_in64 = d_in[:n64].double()
         d_out64 = torch.empty((n64, 5, 16, 16, 16), dtype=torch.float64, device=device)
-        d_scr = torch.empty(hydro.gamer_hydro_f64_scratch_doubles(), dtype=torch.float64, device=device)
         for _ in range(2):
-            hydro.gamer_hydro_advance_f64(d_in64, d_out64, n64, 3, dt, dh, gamma, d_scr, stream=stream)
+            hydro.gamer_hydro_advance_f64_ex(d_in64, d_out64, n64, 3, dt, dh, gamma, stream=stream)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(5):
-            hydro.gamer_hydro_advance_f64(d_in64, d_out64, n64, 3, dt, dh, gamma, d_scr, stream=stream)
+            hydro.gamer_hydro_advance_f64_ex(d_in64, d_out64, n64, 3, dt, dh, gamma, stream=stream)
         e1.record(stream)
         torch.cuda.synchronize()
         ms64 = e0.elapsed_time(e1) / 5
         gbs64 = n64 * 2 * BYTES_PER_GROUP / (ms64 * 1e-3) / 1e9
         e0.record(stream)
         for _ in range(3):
-            hydro.gamer_hydro_advance_f64(d_in64, d_out64, n64, 3, dt, dh, gamma, d_scr, backward=1, stream=stream)
+            hydro.gamer_hydro_advance_f64_ex(d_in64, d_out64, n64, 3, dt, dh, gamma, backward=1, stream=stream)
         e1.record(stream)
         torch.cuda.synchronize()
         ms64b = e0.elapsed_time(e1) / 3
@@ -490,12 +531,12 @@ def run_ours(args):
         torch.cuda.synchronize()
         ms64_opt = eo0.elapsed_time(eo1) / 3
         del d_face64, d_spd64
-        f64 = dict(api="gamer_hydro_advance_f64", n_groups=n64, ns_per_group=ms64 * 1e6 / n64,
+        f64 = dict(api="gamer_hydro_advance_f64_ex", n_groups=n64, ns_per_group=ms64 * 1e6 / n64,
                    ns_per_group_with_face_flux_and_maxspeed=ms64_opt * 1e6 / n64,
                    backward_ns_per_group=ms64b * 1e6 / n64,
                    value=n64 * CELLS_PER_GROUP / (ms64 * 1e-3), unit=UNIT, dtype="f64",
                    hbm_achieved_gbs=gbs64, hbm_frac=gbs64 / peaks["hbm_gbs"], algorithmic_bytes=n64 * 2 * BYTES_PER_GROUP)
-        del d_in64, d_out64, d_scr
+        del d_in64, d_out64
 
     # NEXT-3 (reported separately, not part of the step): device-side ghost fill of the same batch seen as a periodic
     # box of groups — reads every interior once, writes every padded group once.  It overwrites d_in, so it runs last.
@@ -516,6 +557,23 @@ def run_ours(args):
         ghost_fill = dict(api="gamer_hydro_ghost_fill", box_groups=list(box), ms=gf_ms, bound="hbm", achieved=gf_gbs,
                           peak=peaks["hbm_gbs"], unit="GB/s", frac=gf_gbs / peaks["hbm_gbs"],
                           algorithmic_bytes=n * BYTES_PER_GROUP)
+
+        # a thin box: 1024 groups as 256 x 4 x 1 give 20 strips, far fewer than SMs; the walk along x
+        # is cut into segments so that the launch still fills the GPU
+        if n >= 1024:
+            tb = (256, 4, 1)
+            for _ in range(2):
+                hydro.gamer_hydro_ghost_fill(d_out, d_in, tb[0], tb[1], tb[2], stream=stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(5):
+                hydro.gamer_hydro_ghost_fill(d_out, d_in, tb[0], tb[1], tb[2], stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            tb_ms = e0.elapsed_time(e1) / 5
+            ghost_fill["thin_box"] = dict(box_groups=list(tb), ms=tb_ms, achieved=1024 * BYTES_PER_GROUP / (tb_ms * 1e-3) / 1e9,
+                                          unit="GB/s", note="302 MB: partly L2-resident, compare with itself across rounds")
+            hydro.gamer_hydro_ghost_fill(d_out, d_in, box[0], box[1], box[2], stream=stream)   # restore the full box
 
     # NEXT-3 driver: whole steps (dt, forward pass, ghost fill) without leaving the device; runs last, it evolves d_in
     run_uniform = None
@@ -575,6 +633,8 @@ def main():
     ap.add_argument("--streams", type=int, default=3, help="pipeline: number of streams (N_s)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
+    ap.add_argument("--no-pipeline-sweep", action="store_true",
+                    help="skip the pipeline's own report (link rates, N_g x N_s sweep) inside the e2e leg")
     ap.add_argument("--no-check", action="store_true")
     ap.add_argument("--no-config4", action="store_true", help="skip the config-4 sub-record")
     ap.add_argument("--no-ghost-fill", action="store_true", help="skip the separate ghost-fill measurement")

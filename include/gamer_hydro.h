@@ -26,6 +26,13 @@
  * reduction; gamer_hydro_run_uniform does), and nothing applies a density or pressure floor (the
  * paper names none): non-physical input (rho <= 0 or P <= 0) yields NaN/Inf in the affected cells, silently.
  *
+ * NUMBER RANGE (fp32 passes): reciprocals and square roots are the hardware approximations with flush-to-zero
+ * (rcp.approx.ftz, sqrt.approx.ftz; about 1 ulp, the parity bars of DESIGN.md hold with them): a DENORMAL operand or
+ * result of those two operations is taken as zero.  That touches densities above about 8.5e37 (1/rho would be
+ * denormal: it becomes 0, and velocity and pressure with it) and specific internal energies gamma (gamma-1) e_int/rho
+ * below about 1.2e-38 (the sound speed becomes 0).  The CPU oracle keeps denormals, so parity with it is claimed on the
+ * normal range only; every workload of BASELINE.json lies many decades inside it.  The fp64 passes do not flush.
+ *
  * OWNERSHIP: the caller owns every buffer.  `d_*` are DEVICE pointers (cudaMalloc or equivalent) valid on the
  * device of `stream`; `h_*` are HOST pointers.  Nothing is allocated, freed or synchronised by gamer_hydro_advance*:
  * they only enqueue work on `stream` (NULL = the legacy default stream).  `d_in` is never written.  Input, outputs
@@ -168,42 +175,34 @@ GAMER_API long long gamer_hydro_noalloc_max_groups(void);
  * d_face_flux [g][3][3][5][16][16] and d_group_maxspeed [g] are the optional outputs of gamer_hydro_advance_ex in
  * double (NULL = off).  Reciprocals and square roots are accurate to about 1 ulp.  A padded group does not fit in
  * shared memory in double precision: the pass is cut into halves and the rows of the last sweep wait in tensor memory
- * (DESIGN.md 8c); no device scratch is needed. */
+ * (DESIGN.md 8c); no device scratch is needed.
+ * TENSOR MEMORY IS HELD EXCLUSIVELY: each persistent CTA of these kernels allocates all 512 tensor-memory columns of
+ * its SM (tcgen05.alloc, which blocks until they are free) and keeps them until the kernel ends.  Anything else that
+ * uses tensor memory on the same GPU at the same time — a cuBLAS / CUTLASS GEMM of the same process on another
+ * stream — waits for this kernel to finish on the SMs it occupies, or makes this kernel wait for it.  Do not overlap
+ * the fp64 passes with tensor-core GEMMs if either is latency critical.  (The fp32 passes use no tensor memory.)
+ * A device that offers less than 225 408 B of shared memory per block -> GAMER_EUNSUPPORTED. */
 GAMER_API int gamer_hydro_advance_f64_ex(const double* d_in, double* d_out, long long n_groups, int ghost,
                             double dt, double dh, double gamma, int backward, double* d_face_flux,
                             double* d_group_maxspeed, void* stream);
-/* The same without optional outputs.  d_scratch is ignored (round 1 needed gamer_hydro_f64_scratch_doubles() doubles
- * of device scratch; the function now returns 0) and may be NULL. */
-GAMER_API int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost,
-                            double dt, double dh, double gamma, int backward, double* d_scratch, void* stream);
-GAMER_API size_t gamer_hydro_f64_scratch_doubles(void);
 
 /* Launch geometry the library will use on the current device, for reporting: any pointer may be NULL.
  * grid = number of persistent CTAs for n_groups, block = threads per CTA, smem = dynamic shared memory per CTA in
  * bytes, regs = registers per thread of the kernel. */
 GAMER_API int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread);
 
-/* Measurement aid for the roofline: an FMA-only micro-benchmark of the FP32 pipe of the current
- * device — 4 CTAs of 512 threads per SM, 16 independent fused multiply-add chains per thread, 2048 steps each —
- * launched repeats + 1 times on the default stream (the first is a warm-up), timed with CUDA events; SYNCHRONOUS.
- * *tflops receives the best launch's 2 x FMA count / time in TFLOP/s; *lane_fma_per_clk_per_sm (optional) the same as
- * FMAs per clock per SM if sm_mhz (the SM clock the caller observed, MHz) is > 0 — 128 is the unit count of the part.
- * d_sink: one float of device memory (never written in practice).  Not part of the hydro path. */
-GAMER_API int gamer_hydro_fp32_peak(int repeats, float* d_sink, double* tflops, double* lane_fma_per_clk_per_sm,
-                          double sm_mhz);
-
-/* Measurement aid for DESIGN.md 7 (why the pass is bound by instruction issue and register-file reads), SYNCHRONOUS,
- * allocates and frees its own few hundred KB of device memory; not part of the hydro path.
- *   what = 0: *cycles = clocks one SM sub-partition needs per warp-wide FMA whose three source operands are three
- *             different registers (an FMA with two reused operands takes 1.05), 4 warps per sub-partition;
- *   what = 1, 2, 3: *cycles = clocks per warp-march (one warp, 32 rows of 22 cells, the production row march along x, y,
- *             z) and sub-partition slot when warps_per_smsp = 1..4 warps per sub-partition run marches back to back
- *             on a resident group with no loads and no barriers — the steady-state cost a schedule can at best reach.
- * Values are means over the SMs of the current device, read from clock64 inside the kernels. */
-GAMER_API int gamer_hydro_issue_probe(int what, int warps_per_smsp, double* cycles);
-
 GAMER_API const char* gamer_last_error(void);   /* thread-local, static storage; "" if the last call on this thread succeeded */
 GAMER_API const char* gamer_version(void);      /* static string */
+
+/* Binary-interface revision of the library that is loaded; compare with GAMER_HYDRO_ABI_VERSION of the header you
+ * compiled against and refuse to run on a mismatch.  It is bumped whenever an exported function changes its argument
+ * list or is removed: a caller built against an older header would still link and would silently pass shifted
+ * arguments.  History: 1 = round 1; 2 = gamer_hydro_run_uniform gained `order` (between n_steps and cfl);
+ * 3 = gamer_hydro_advance_f64 and gamer_hydro_f64_scratch_doubles removed (use gamer_hydro_advance_f64_ex with NULL
+ * optional outputs; no device scratch exists any more), the measurement probes moved to libgamer_probes
+ * (include/gamer_probes.h), gamer_hydro_run_uniform_noalloc added. */
+#define GAMER_HYDRO_ABI_VERSION 3
+GAMER_API int gamer_hydro_abi_version(void);
 
 #ifdef __cplusplus
 }

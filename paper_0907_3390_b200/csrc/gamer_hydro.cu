@@ -55,6 +55,7 @@ KernelFn pick_kernel(bool backward, bool face, bool speed) {
 struct DeviceInfo {
     bool ready = false;
     int sm_count = 0;
+    int smem_optin = 0;          // dynamic shared memory a block may opt in to, bytes
     bool attr_set[32] = {};      // one flag per kernel key (prepare())
 };
 std::mutex g_mu;
@@ -80,7 +81,7 @@ int prepare(const void* fn, int key, int smem_bytes, int* sm_count) {
     std::lock_guard<std::mutex> lk(g_mu);
     DeviceInfo& di = g_dev[dev];
     if (!di.ready) {
-        int major = 0, smem_optin = 0;
+        int major = 0, smem_optin = 0;      // (checked per kernel below: the fp64 kernels need more than the fp32 ones)
         e = cudaDeviceGetAttribute(&di.sm_count, cudaDevAttrMultiProcessorCount, dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
@@ -91,9 +92,13 @@ int prepare(const void* fn, int key, int smem_bytes, int* sm_count) {
         if (smem_optin < gamer::SMEM_BYTES)
             return fail(GAMER_EUNSUPPORTED, "device offers %d B of shared memory per block, %d needed", smem_optin,
                         gamer::SMEM_BYTES);
+        di.smem_optin = smem_optin;
         di.ready = true;
     }
     if (!di.attr_set[key]) {
+        if (smem_bytes > di.smem_optin)
+            return fail(GAMER_EUNSUPPORTED, "device %d offers %d B of shared memory per block, this kernel needs %d", dev,
+                        di.smem_optin, smem_bytes);
         e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
         if (e != cudaSuccess) return fail(GAMER_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e));
         di.attr_set[key] = true;
@@ -127,19 +132,7 @@ int check_disjoint(const void* const* ptr, const size_t* bytes, int n) {
     return GAMER_OK;
 }
 
-gamer::GasConst make_const(float dt, float dh, float gamma) {
-    gamer::GasConst gc;
-    const float k = dt / dh;
-    gc.gm1 = gamma - 1.0f;
-    gc.ggm1 = gamma * (gamma - 1.0f);
-    gc.kq = 0.25f * k;
-    gc.kh = 0.5f * k;
-    gc.dh = dh;
-    gc.sg = sqrtf(gc.ggm1);
-    gc.kq_gm1 = gc.kq * gc.gm1;
-    gc.kq_sg = gc.kq * gc.sg;
-    return gc;
-}
+using gamer::make_const;
 
 int launch(const float* d_in, float* d_out, long long n_groups, float dt, float dh, float gamma, int backward,
            float* d_face, float* d_speed, cudaStream_t stream) {
@@ -154,86 +147,6 @@ int launch(const float* d_in, float* d_out, long long n_groups, float dt, float 
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "kernel launch: %s", cudaGetErrorString(e));
     return GAMER_OK;
-}
-
-// FMA-only micro-benchmark of the FP32 pipe ("measures an FMA-only micro-benchmark, and states which
-// number is used"): 16 independent FFMA chains per thread, nothing else in the loop but its counter.
-constexpr int PEAK_CHAINS = 16, PEAK_ITERS = 2048, PEAK_THREADS = 512, PEAK_CTAS_PER_SM = 4;
-__global__ void __launch_bounds__(PEAK_THREADS) fp32_peak_kernel(float* __restrict__ sink, float a, float b) {
-    float x[PEAK_CHAINS];
-#pragma unroll
-    for (int i = 0; i < PEAK_CHAINS; ++i) x[i] = 1e-3f * (float)(threadIdx.x + i);
-    const float m = a + 1e-9f * (float)(threadIdx.x & 1), c = b;      // per-thread values: stay in vector registers
-#pragma unroll 8
-    for (int it = 0; it < PEAK_ITERS; ++it) {
-#pragma unroll
-        for (int i = 0; i < PEAK_CHAINS; ++i) x[i] = fmaf(x[i], m, c);
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < PEAK_CHAINS; ++i) s += x[i];
-    if (s == 123.456f) sink[0] = s;                                    // keeps the chains alive, never true in practice
-}
-
-// Issue-rate probes: what an SM sub-partition sustains on the instruction mix of this kernel.
-//   ffma3_probe_kernel: fused multiply-adds whose three source operands are three different registers that no
-//     neighbouring instruction shares (the register file delivers about two operands per clock to a sub-partition:
-//     such an FMA costs 1.5 issue slots, one with two reused operands costs 1).
-//   march_probe_kernel<D>: the production row march (rtvd_march.cuh, the sweep of hydro_kernel.cuh along axis D) back to
-//     back on k warps per sub-partition, in place on one resident group, no loads, no barriers: cycles per warp-march.
-constexpr int PROBE3_CHAINS = 16, PROBE3_ITERS = 2000;
-__global__ void __launch_bounds__(512, 1) ffma3_probe_kernel(float* __restrict__ sink, long long* __restrict__ cyc) {
-    float x[PROBE3_CHAINS], y[PROBE3_CHAINS], z[PROBE3_CHAINS];
-#pragma unroll
-    for (int i = 0; i < PROBE3_CHAINS; ++i) {
-        x[i] = threadIdx.x * 1e-3f + i;
-        y[i] = 1.0f + 1e-6f * (threadIdx.x + i);
-        z[i] = 1e-7f * (threadIdx.x + 3 * i);
-    }
-    const long long t0 = clock64();
-#pragma unroll 1
-    for (int it = 0; it < PROBE3_ITERS; ++it) {
-#pragma unroll
-        for (int r = 0; r < 4; ++r)
-#pragma unroll
-            for (int i = 0; i < PROBE3_CHAINS; ++i) x[i] = fmaf(x[i], y[i], z[i]);
-    }
-    const long long t1 = clock64();
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < PROBE3_CHAINS; ++i) s += x[i] + y[i] + z[i];
-    if (s == 123.456f) sink[0] = s;
-    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned long long*>(&cyc[blockIdx.x]), (unsigned long long)(t1 - t0));
-}
-
-template <int D>
-__global__ void __launch_bounds__(gamer::BLOCK_THREADS, 1)
-march_probe_kernel(const float* __restrict__ in, gamer::GasConst gc, int k_per_smsp, int reps, long long* __restrict__ cyc,
-                   float* __restrict__ sink) {
-    using namespace gamer;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    float* smem = reinterpret_cast<float*>(smem_raw);
-    for (int i = threadIdx.x; i < GROUP_IN_FLOATS; i += blockDim.x) smem[i] = in[i];
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    NoGate nogate;
-    float speed = 0.f;
-    const long long t0 = clock64();
-    if (warp < 4 * k_per_smsp) {
-#pragma unroll 1
-        for (int r = 0; r < reps; ++r) {
-            // rows are shared between warps where a sweep has fewer than 512: same values, timing only
-            if (D == 0)
-                sweep<0, 0, NP, 0, NP, false, false, false, false>(smem, gc, nullptr, nullptr, speed, (32 * warp + lane) % 480, nogate);
-            else if (D == 1)
-                sweep<1, NG, PS, 0, NP, false, false, false, false>(smem, gc, nullptr, nullptr, speed, ((threadIdx.x % 352) & ~31) | lane, nogate);
-            else
-                sweep<2, NG, PS, NG, PS, false, false, false, false>(smem, gc, nullptr, nullptr, speed, threadIdx.x % 256, nogate);
-        }
-    }
-    const long long t1 = clock64();
-    if (lane == 0) atomicMax(reinterpret_cast<unsigned long long*>(&cyc[blockIdx.x]), (unsigned long long)(t1 - t0));
-    if (smem[12345] == 123.456f) sink[0] = smem[12345] + speed;
 }
 
 }  // namespace
@@ -407,7 +320,7 @@ int gamer_hydro_pipeline_release(void) {
 
 static int check_box(int gx, int gy, int gz, int bc_x, int bc_y, int bc_z) {
     if (gx < 1 || gy < 1 || gz < 1) return fail(GAMER_EINVAL, "box of %d x %d x %d groups", gx, gy, gz);
-    if (gamer::ghost_fill_ctas(gx, gy, gz) > (1ll << 31) - 1) return fail(GAMER_EINVAL, "too many groups for one launch");
+    if ((long long)gx * gy * gz * gamer::NCOMP > (1ll << 31) - 1) return fail(GAMER_EINVAL, "too many groups for one launch");
     if ((bc_x | bc_y | bc_z) & ~1) return fail(GAMER_EINVAL, "boundary flags must be 0 (periodic) or 1 (keep)");
     return GAMER_OK;
 }
@@ -422,8 +335,8 @@ int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int
     int sm_count = 0;
     rc = prepare(reinterpret_cast<const void*>(gamer::ghost_fill_kernel), 13, gamer::GF_SMEM_BYTES, &sm_count);
     if (rc != GAMER_OK) return rc;
-    gamer::BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
-    gamer::ghost_fill_kernel<<<(unsigned int)gamer::ghost_fill_ctas(gx, gy, gz), gamer::GF_THREADS, gamer::GF_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(
+    gamer::BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}, gamer::ghost_fill_segments(gx, gy, gz, sm_count)};
+    gamer::ghost_fill_kernel<<<(unsigned int)gamer::ghost_fill_ctas(gx, gy, gz, geo.nseg), gamer::GF_THREADS, gamer::GF_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(
         d_interior, d_padded, geo);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "ghost_fill launch: %s", cudaGetErrorString(e));
@@ -464,7 +377,8 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     const int grid = (int)(n < (long long)sm_count ? n : (long long)sm_count);
     const int red_grid = (int)(n < 4ll * sm_count ? n : 4ll * sm_count);
     const unsigned int gsm_grid = (unsigned int)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024);
-    BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}};
+    BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}, ghost_fill_segments(gx, gy, gz, sm_count)};
+    const unsigned int gf_grid = (unsigned int)ghost_fill_ctas(gx, gy, gz, geo.nseg);
     unsigned int* acc = reinterpret_cast<unsigned int*>(d_work);
     float* d_speed = d_work + 4;
     // Eq.30 over ALL padded cells (reading R10) costs one pass over the initial state.  After that the padded state
@@ -481,11 +395,11 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
         fwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr,
                                                          order == 0 ? d_speed : nullptr, d_work + 1);
         if (order == 1) {       // the backward sweep z,y,x follows with the SAME time step
-            ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
+            ghost_fill_kernel<<<gf_grid, GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
             bwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr, d_speed, d_work + 1);
         }
         group_speed_max_kernel<<<gsm_grid, 256, 0, stream>>>(d_speed, n, acc);
-        ghost_fill_kernel<<<(unsigned int)ghost_fill_ctas(gx, gy, gz), GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
+        ghost_fill_kernel<<<gf_grid, GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "run_uniform: %s", cudaGetErrorString(e));
@@ -516,8 +430,6 @@ int gamer_hydro_run_uniform_noalloc(float* d_padded, float* d_interior, int gx, 
     return gamer_hydro_run_uniform(d_padded, d_interior, gx, gy, gz, bc_x, bc_y, bc_z, n_steps, order, cfl, dh, gamma,
                                    d_work, d_dt_log, stream);
 }
-
-size_t gamer_hydro_f64_scratch_doubles(void) { return 0; }      // round 1 passed rows through device memory; tensor memory now
 
 int gamer_hydro_advance_f64_ex(const double* d_in, double* d_out, long long n_groups, int ghost, double dt, double dh,
                                double gamma, int backward, double* d_face_flux, double* d_group_maxspeed, void* stream) {
@@ -564,12 +476,6 @@ int gamer_hydro_advance_f64_ex(const double* d_in, double* d_out, long long n_gr
     return GAMER_OK;
 }
 
-int gamer_hydro_advance_f64(const double* d_in, double* d_out, long long n_groups, int ghost, double dt, double dh,
-                            double gamma, int backward, double* d_scratch, void* stream) {
-    (void)d_scratch;          // no longer used (any value, NULL included)
-    return gamer_hydro_advance_f64_ex(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward, nullptr, nullptr, stream);
-}
-
 int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem_bytes, int* regs_per_thread) {
     const void* fn = reinterpret_cast<const void*>(pick_kernel(false, false, false));
     const int smem = gamer::SMEM_BYTES;
@@ -588,87 +494,8 @@ int gamer_hydro_launch_info(long long n_groups, int* grid, int* block, int* smem
     return GAMER_OK;
 }
 
-int gamer_hydro_fp32_peak(int repeats, float* d_sink, double* tflops, double* lane_fma_per_clk_per_sm, double sm_mhz) {
-    if (repeats < 1 || d_sink == nullptr || tflops == nullptr) return fail(GAMER_EINVAL, "repeats >= 1, d_sink and tflops non-NULL");
-    int dev = 0, sm = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(GAMER_ECUDA, "no CUDA device: %s", cudaGetErrorString(e)); }
-    cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(GAMER_ECUDA, "cudaEventCreate");
-    const int grid = sm * PEAK_CTAS_PER_SM;
-    double best_ms = 1e30;
-    for (int r = 0; r < repeats + 1 && e == cudaSuccess; ++r) {           // the first launch is a warm-up
-        cudaEventRecord(e0, 0);
-        fp32_peak_kernel<<<grid, PEAK_THREADS>>>(d_sink, 1.0000001f, 1e-7f);
-        cudaEventRecord(e1, 0);
-        e = cudaEventSynchronize(e1);
-        float ms = 0.f;
-        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-        if (r > 0 && ms < best_ms) best_ms = ms;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (e != cudaSuccess) return fail(GAMER_ECUDA, "fp32_peak: %s", cudaGetErrorString(e));
-    const double fma = (double)grid * PEAK_THREADS * PEAK_CHAINS * PEAK_ITERS;
-    *tflops = 2.0 * fma / (best_ms * 1e-3) / 1e12;
-    if (lane_fma_per_clk_per_sm) *lane_fma_per_clk_per_sm = sm_mhz > 0 ? fma / (best_ms * 1e-3) / (sm_mhz * 1e6) / sm : 0.0;
-    g_err[0] = '\0';
-    return GAMER_OK;
-}
-
-int gamer_hydro_issue_probe(int what, int warps_per_smsp, double* cycles) {
-    if (cycles == nullptr || what < 0 || what > 3 || warps_per_smsp < 1 || warps_per_smsp > 4)
-        return fail(GAMER_EINVAL, "issue_probe: what in 0..3, warps_per_smsp in 1..4, cycles non-NULL");
-    int sm_count = 0;
-    int rc = prepare(reinterpret_cast<const void*>(march_probe_kernel<0>), 17, gamer::SMEM_BYTES, &sm_count);
-    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(march_probe_kernel<1>), 18, gamer::SMEM_BYTES, &sm_count);
-    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(march_probe_kernel<2>), 19, gamer::SMEM_BYTES, &sm_count);
-    if (rc != GAMER_OK) return rc;
-    // one group of a smooth, physical, non-uniform state; a tiny dt/dh keeps it so over the in-place repetitions
-    std::vector<float> h(gamer::GROUP_IN_FLOATS);
-    unsigned int seed = 12345u;
-    for (int v = 0; v < gamer::NCOMP; ++v)
-        for (int i = 0; i < gamer::VAR_FLOATS; ++i) {
-            seed = seed * 1664525u + 1013904223u;
-            const float r = (float)(seed >> 8) * (1.0f / 16777216.0f);
-            h[(size_t)v * gamer::VAR_FLOATS + i] = v == 0 ? 1.f + 0.1f * r : (v == 4 ? 1.5f + 0.1f * r : 0.1f * (r - 0.5f));
-        }
-    float* d_in = nullptr;
-    long long* d_cyc = nullptr;
-    float* d_sink = nullptr;
-    cudaError_t e = cudaMalloc(&d_in, gamer::GROUP_IN_BYTES);
-    if (e == cudaSuccess) e = cudaMalloc(&d_cyc, (size_t)sm_count * sizeof(long long));
-    if (e == cudaSuccess) e = cudaMalloc(&d_sink, sizeof(float));
-    if (e == cudaSuccess) e = cudaMemcpy(d_in, h.data(), gamer::GROUP_IN_BYTES, cudaMemcpyHostToDevice);
-    const int reps = 20;
-    gamer::GasConst gc = make_const(0.01f, 1.0f, 5.0f / 3.0f);
-    std::vector<long long> c(sm_count);
-    for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {          // the first pass is a warm-up
-        e = cudaMemset(d_cyc, 0, (size_t)sm_count * sizeof(long long));
-        if (e != cudaSuccess) break;
-        if (what == 0) ffma3_probe_kernel<<<sm_count, 512>>>(d_sink, d_cyc);
-        else if (what == 1) march_probe_kernel<0><<<sm_count, gamer::BLOCK_THREADS, gamer::SMEM_BYTES>>>(d_in, gc, warps_per_smsp, reps, d_cyc, d_sink);
-        else if (what == 2) march_probe_kernel<1><<<sm_count, gamer::BLOCK_THREADS, gamer::SMEM_BYTES>>>(d_in, gc, warps_per_smsp, reps, d_cyc, d_sink);
-        else march_probe_kernel<2><<<sm_count, gamer::BLOCK_THREADS, gamer::SMEM_BYTES>>>(d_in, gc, warps_per_smsp, reps, d_cyc, d_sink);
-        e = cudaDeviceSynchronize();
-        if (e == cudaSuccess) e = cudaMemcpy(c.data(), d_cyc, (size_t)sm_count * sizeof(long long), cudaMemcpyDeviceToHost);
-    }
-    cudaFree(d_in);
-    cudaFree(d_cyc);
-    cudaFree(d_sink);
-    if (e != cudaSuccess) { (void)cudaGetLastError(); return fail(GAMER_ECUDA, "issue_probe: %s", cudaGetErrorString(e)); }
-    double mean = 0.0;
-    for (int i = 0; i < sm_count; ++i) mean += (double)c[i];
-    mean /= sm_count;
-    // what = 0: 4 warps per sub-partition (512 threads), cycles per warp instruction of one sub-partition;
-    // what = 1..3: cycles per warp-march and sub-partition slot
-    *cycles = what == 0 ? mean / (4.0 * PROBE3_ITERS * 4 * PROBE3_CHAINS) : mean / reps / warps_per_smsp;
-    g_err[0] = '\0';
-    return GAMER_OK;
-}
-
 const char* gamer_last_error(void) { return g_err; }
-const char* gamer_version(void) { return "gamer-hydro-b200 0.1.0 (sm_100a)"; }
+const char* gamer_version(void) { return "gamer-hydro-b200 0.3.0 (sm_100a)"; }
+int gamer_hydro_abi_version(void) { return GAMER_HYDRO_ABI_VERSION; }
 
 }  // extern "C"

@@ -71,7 +71,7 @@ struct SmemSink {
     template <int P>
     __device__ __forceinline__ void cell(int j, const float (&u)[NCOMP]) {
         constexpr int ODD = P & 1;
-        if (STRIDE == 1 && !GAMER_X32) {
+        if (STRIDE == 1) {
             if (ODD) {
                 if (j == NG) {
 #pragma unroll
@@ -137,7 +137,7 @@ struct FinalSink {
         } else if (TO_GLOBAL) {
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) dst[k][(j - NG) * OSTRIDE] = u[k];
-        } else if (STRIDE == 1 && !GAMER_X32) {
+        } else if (STRIDE == 1) {
             if (ODD) {
                 if (j == NG) {
 #pragma unroll

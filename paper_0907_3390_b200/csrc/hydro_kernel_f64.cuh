@@ -29,13 +29,7 @@ constexpr int F64_THREADS = 256;
 constexpr int HALF_PLANES = NP / 2;                                  // 11
 constexpr int HALF_VAR = HALF_PLANES * NP * NP;                      // 5324 doubles: one variable of a half
 constexpr int ZBUF_VAR = NP * PS * PS;                               // 5632 doubles: one variable of the z-sweep block
-constexpr int BWD_VAR = PS * NP * NP;                                // 7744 doubles: 16 z-swept planes of one variable
-constexpr int BWD_SCRATCH_DOUBLES = NCOMP * BWD_VAR;                 // 38 720 per CTA (backward pass)
-constexpr int BWD_CHUNK_PLANES = 8;                                  // planes per y/x stage of the backward pass
-constexpr int BWD_CHUNK_VAR = BWD_CHUNK_PLANES * NP * NP;            // 3872
-constexpr int FWD_SCRATCH_DOUBLES = NCOMP * ZBUF_VAR;                // 28 160 per CTA (forward pass)
-constexpr int F64_SCRATCH_DOUBLES = BWD_SCRATCH_DOUBLES;             // what the caller provides per CTA
-constexpr int F64_DATA_BYTES = FWD_SCRATCH_DOUBLES * 8;              // 225 280 (>= 5 * 5324 * 8 = 212 960)
+constexpr int F64_DATA_BYTES = NCOMP * ZBUF_VAR * 8;                 // 225 280 (>= 5 * 5324 * 8 = 212 960)
 constexpr int F64_SMEM_BYTES = F64_DATA_BYTES + 128;     // + mbarrier, TMEM base address, 8 doubles of reduction scratch
 
 

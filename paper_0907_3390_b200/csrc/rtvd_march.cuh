@@ -22,10 +22,6 @@
 #define GAMER_MARCH_UNROLL 3     /* pairs of cells per loop body (measured: 1: 113.5, 2: 105.4, 3: 104.5, 4: 108.4 ns/group) */
 #endif
 
-#ifndef GAMER_X32
-#define GAMER_X32 0       /* experiment: 32-bit shared-memory accesses along x */
-#endif
-
 #ifndef GAMER_MARCH_UNROLL_F64
 #define GAMER_MARCH_UNROLL_F64 2       /* pairs per body in fp64 (measured: 1: 294, 2: 288, 3: 481 ns/group forward) */
 #endif
@@ -52,6 +48,21 @@ struct GasConstT {
     T sg;       // sqrt(gamma (gamma-1)) }
 };
 using GasConst = GasConstT<float>;
+
+// the constants of one pass, formed on the host in fp32 (the kernels that read dt from device memory repeat exactly this)
+inline GasConst make_const(float dt, float dh, float gamma) {
+    GasConst gc;
+    const float k = dt / dh;
+    gc.gm1 = gamma - 1.0f;
+    gc.ggm1 = gamma * (gamma - 1.0f);
+    gc.kq = 0.25f * k;
+    gc.kh = 0.5f * k;
+    gc.dh = dh;
+    gc.sg = sqrtf(gc.ggm1);
+    gc.kq_gm1 = gc.kq * gc.gm1;
+    gc.kq_sg = gc.kq * gc.sg;
+    return gc;
+}
 
 // explicitly rounded (never contracted) operations and fused multiply-add, per precision
 __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
@@ -322,7 +333,7 @@ template <int STRIDE>
 struct StrideSrc {
     const float* src[NCOMP];
     __device__ __forceinline__ void load(int n, float (&ua)[NCOMP], float (&ub)[NCOMP]) const {
-        if (STRIDE == 1 && !GAMER_X32) {
+        if (STRIDE == 1) {
 #pragma unroll
             for (int k = 0; k < NCOMP; ++k) {
                 const float2 t = *reinterpret_cast<const float2*>(src[k] + n);

@@ -32,6 +32,10 @@ def lib():
             raise ImportError("%s not found: build it with `python -m paper_0907_3390_b200.build` "
                               "(there is no CPU fallback)" % LIB_PATH)
         L = ctypes.CDLL(LIB_PATH)
+        L.gamer_hydro_abi_version.restype = ctypes.c_int
+        if L.gamer_hydro_abi_version() != ABI_VERSION:
+            raise ImportError("%s has ABI version %d, this binding needs %d: rebuild it"
+                              % (LIB_PATH, L.gamer_hydro_abi_version(), ABI_VERSION))
         vp, ll, ci, cf = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_float
         L.gamer_hydro_advance.restype = ci
         L.gamer_hydro_advance.argtypes = [vp, vp, ll, ci, cf, cf, cf, vp]
@@ -55,23 +59,16 @@ def lib():
         L.gamer_hydro_run_uniform_noalloc.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, ci, cf, cf, cf, vp, vp]
         L.gamer_hydro_noalloc_max_groups.restype = ll
         L.gamer_hydro_noalloc_max_groups.argtypes = []
-        L.gamer_hydro_advance_f64.restype = ci
-        L.gamer_hydro_advance_f64.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp]
         L.gamer_hydro_advance_f64_ex.restype = ci
         L.gamer_hydro_advance_f64_ex.argtypes = [vp, vp, ll, ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, vp, vp, vp]
-        L.gamer_hydro_f64_scratch_doubles.restype = ctypes.c_size_t
-        L.gamer_hydro_f64_scratch_doubles.argtypes = []
         L.gamer_hydro_launch_info.restype = ci
         L.gamer_hydro_launch_info.argtypes = [ll] + [ctypes.POINTER(ci)] * 4
-        L.gamer_hydro_fp32_peak.restype = ci
-        L.gamer_hydro_fp32_peak.argtypes = [ci, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
-                                            ctypes.c_double]
-        L.gamer_hydro_issue_probe.restype = ci
-        L.gamer_hydro_issue_probe.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double)]
         L.gamer_last_error.restype = ctypes.c_char_p
         L.gamer_last_error.argtypes = []
         L.gamer_version.restype = ctypes.c_char_p
         L.gamer_version.argtypes = []
+        L.gamer_hydro_abi_version.restype = ci
+        L.gamer_hydro_abi_version.argtypes = []
         _lib = L
     return _lib
 
@@ -109,6 +106,13 @@ def gamer_last_error():
 
 def gamer_version():
     return lib().gamer_version().decode()
+
+
+ABI_VERSION = 3          # GAMER_HYDRO_ABI_VERSION of the header this binding was written against
+
+
+def gamer_hydro_abi_version():
+    return int(lib().gamer_hydro_abi_version())
 
 
 def gamer_hydro_in_floats(n_groups, ghost=NGHOST):
@@ -196,20 +200,6 @@ def gamer_hydro_noalloc_max_groups():
     return int(lib().gamer_hydro_noalloc_max_groups())
 
 
-def gamer_hydro_f64_scratch_doubles():
-    return int(lib().gamer_hydro_f64_scratch_doubles())
-
-
-def gamer_hydro_advance_f64(d_in, d_out, n_groups, ghost, dt, dh, gamma, d_scratch, backward=0, stream=None,
-                            check=True):
-    """One pass in double precision; d_scratch: gamer_hydro_f64_scratch_doubles() doubles."""
-    rc = lib().gamer_hydro_advance_f64(_ptr(d_in), _ptr(d_out), n_groups, ghost, dt, dh, gamma, int(backward),
-                                       _ptr(d_scratch), _stream_ptr(stream))
-    if check:
-        _check(rc)
-    return rc
-
-
 def gamer_hydro_advance_f64_ex(d_in, d_out, n_groups, ghost, dt, dh, gamma, backward=0, d_face_flux=None,
                                d_group_maxspeed=None, stream=None, check=True):
     """One pass in double precision with the optional outputs (face fluxes, per-group CFL speed) in double."""
@@ -220,21 +210,7 @@ def gamer_hydro_advance_f64_ex(d_in, d_out, n_groups, ghost, dt, dh, gamma, back
     return rc
 
 
-def gamer_hydro_fp32_peak(repeats, d_sink, sm_mhz=0.0):
-    """FMA-only micro-benchmark of the FP32 pipe (measurement aid): returns (TFLOP/s, FMAs per clock per SM)."""
-    t, l = ctypes.c_double(0.0), ctypes.c_double(0.0)
-    _check(lib().gamer_hydro_fp32_peak(int(repeats), _ptr(d_sink), ctypes.byref(t), ctypes.byref(l), float(sm_mhz)))
-    return t.value, l.value
-
-
 def gamer_hydro_launch_info(n_groups):
     g, b, s, r = (ctypes.c_int(0) for _ in range(4))
     _check(lib().gamer_hydro_launch_info(n_groups, ctypes.byref(g), ctypes.byref(b), ctypes.byref(s), ctypes.byref(r)))
     return dict(grid=g.value, block=b.value, smem_bytes=s.value, regs_per_thread=r.value)
-
-
-def gamer_hydro_issue_probe(what, warps_per_smsp=4):
-    """Measurement aid: clocks per 3-register FMA (what = 0) or per warp-march along x, y, z (1, 2, 3)."""
-    c = ctypes.c_double(0.0)
-    _check(lib().gamer_hydro_issue_probe(int(what), int(warps_per_smsp), ctypes.byref(c)))
-    return c.value

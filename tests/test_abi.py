@@ -11,14 +11,14 @@ from paper_0907_3390_b200 import hydro
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    names = []
-    for fn in os.listdir(os.path.join(ROOT, "include")):
-        if fn.endswith(".h"):
-            src = open(os.path.join(ROOT, "include", fn)).read()
-            src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-            names += re.findall(r"GAMER_API\s+[\w\s\*]+?\b(gamer_\w+)\s*\(", src)
-    return sorted(set(names))
+def declared_symbols(header="gamer_hydro.h", macro="GAMER_API"):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(macro + r"\s+[\w\s\*]+?\b(gamer_\w+)\s*\(", src)))
+
+
+def test_every_header_is_covered():
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["gamer_hydro.h", "gamer_probes.h"]
 
 
 def test_header_declares_the_survey_entry_points():
@@ -27,9 +27,29 @@ def test_header_declares_the_survey_entry_points():
               "gamer_hydro_pipeline_run", "gamer_last_error", "gamer_version",
               # beyond the survey's list: NEXT-2 size helper, NEXT-3, NEXT-4, pipeline housekeeping, reporting
               "gamer_hydro_face_flux_floats", "gamer_hydro_ghost_fill", "gamer_hydro_run_uniform",
-              "gamer_hydro_advance_f64", "gamer_hydro_f64_scratch_doubles", "gamer_hydro_pipeline_release",
-              "gamer_hydro_launch_info", "gamer_hydro_fp32_peak"):
+              "gamer_hydro_advance_f64_ex", "gamer_hydro_pipeline_release", "gamer_hydro_launch_info",
+              "gamer_hydro_run_uniform_noalloc", "gamer_hydro_abi_version"):
         assert s in syms
+    # the product ABI is the hydro path: no measurement aid, no dead entry point
+    assert not [s for s in syms if "probe" in s or "peak" in s or "scratch" in s], syms
+
+
+def test_abi_version_matches_the_header():
+    src = open(os.path.join(ROOT, "include", "gamer_hydro.h")).read()
+    v = int(re.search(r"#define\s+GAMER_HYDRO_ABI_VERSION\s+(\d+)", src).group(1))
+    assert hydro.gamer_hydro_abi_version() == v == hydro.ABI_VERSION
+
+
+def test_probe_library_exports_its_header_and_the_product_library_does_not():
+    from paper_0907_3390_b200 import probes
+    hydro.lib()                                   # (skips when the session could not build)
+    P, L = ctypes.CDLL(probes.LIB_PATH), ctypes.CDLL(hydro.LIB_PATH)
+    names = declared_symbols("gamer_probes.h", "GAMER_PROBE_API")
+    assert names == ["gamer_probe_fp32_peak", "gamer_probe_issue", "gamer_probe_last_error"]
+    for s in names:
+        assert hasattr(P, s), s
+        assert not hasattr(L, s), s
+        assert callable(getattr(probes, s, None)), s
 
 
 def test_library_exports_every_declared_symbol():
@@ -103,7 +123,7 @@ def test_overlapping_buffers_are_refused_without_a_device():
     assert refused(L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 1, a_face, a_face + 16, None))
     assert refused(L.gamer_hydro_advance_ex(a_in, a_out, 1, 3, 0.1, 1.0, 1.4, 1, None, a_in + 64, None))
     assert refused(L.gamer_hydro_pipeline_run(a_in, a_in + 1024, 1, 3, 0.1, 1.0, 1.4, 0, 8, 2))
-    assert refused(L.gamer_hydro_advance_f64(a_in, a_in + 64, 1, 3, 0.1, 1.0, 1.4, 0, a_out, None))
+    assert refused(L.gamer_hydro_advance_f64_ex(a_in, a_in + 64, 1, 3, 0.1, 1.0, 1.4, 0, None, None, None))
     # d_work (4 + n floats) inside the padded array; the dt log inside d_work
     assert refused(L.gamer_hydro_run_uniform(a_in, a_out, 1, 1, 1, 0, 0, 0, 1, 0, 0.5, 1.0, 1.4, a_in + 160, None, None))
     assert refused(L.gamer_hydro_run_uniform(a_in, a_out, 1, 1, 1, 0, 0, 0, 4, 1, 0.5, 1.0, 1.4, a_face, a_face + 16, None))
@@ -132,6 +152,9 @@ def test_oracle_and_product_do_not_import_each_other():
 def test_issue_probe_rejects_bad_arguments_without_a_device():
     import ctypes
     c = ctypes.c_double(0.0)
-    assert hydro.lib().gamer_hydro_issue_probe(4, 1, ctypes.byref(c)) == hydro.GAMER_EINVAL
-    assert hydro.lib().gamer_hydro_issue_probe(1, 5, ctypes.byref(c)) == hydro.GAMER_EINVAL
-    assert hydro.lib().gamer_hydro_issue_probe(1, 1, None) == hydro.GAMER_EINVAL
+    from paper_0907_3390_b200 import probes
+    hydro.lib()
+    assert probes.lib().gamer_probe_issue(4, 1, ctypes.byref(c)) == -1
+    assert probes.lib().gamer_probe_issue(1, 5, ctypes.byref(c)) == -1
+    assert probes.lib().gamer_probe_issue(1, 1, None) == -1
+    assert "warps_per_smsp" in probes.gamer_probe_last_error()

@@ -20,16 +20,16 @@ def test_f64_argument_validation_needs_no_device():
     L = hydro.lib()
     buf = (ctypes.c_double * 64)()
     a16 = (ctypes.addressof(buf) + 15) & ~15
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 2, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EUNSUPPORTED
-    assert L.gamer_hydro_advance_f64(a16, a16, -1, 3, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(None, a16, 1, 3, 0.1, 1.0, 1.4, 0, None, None) == hydro.GAMER_EINVAL       # NULL input
+    assert L.gamer_hydro_advance_f64_ex(a16, a16, 1, 2, 0.1, 1.0, 1.4, 0, None, None, None) == hydro.GAMER_EUNSUPPORTED
+    assert L.gamer_hydro_advance_f64_ex(a16, a16, -1, 3, 0.1, 1.0, 1.4, 0, None, None, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64_ex(None, a16, 1, 3, 0.1, 1.0, 1.4, 0, None, None, None) == hydro.GAMER_EINVAL       # NULL input
     assert L.gamer_hydro_advance_f64_ex(a16, a16 + 4259200, 1, 3, 0.1, 1.0, 1.4, 0, a16 + 8, None, None) == hydro.GAMER_EINVAL   # face alignment
     assert L.gamer_hydro_advance_f64_ex(a16, a16 + 4259200, 1, 3, 0.1, 1.0, 1.4, 0, a16 + 16, None, None) == hydro.GAMER_EINVAL  # face overlaps in
-    assert L.gamer_hydro_advance_f64(a16, a16 + 8, 1, 3, 0.1, 1.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL    # alignment
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 0.0, 1.4, 0, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.0, 0, a16, None) == hydro.GAMER_EINVAL
-    assert L.gamer_hydro_advance_f64(a16, a16, 1, 3, 0.1, 1.0, 1.4, 2, a16, None) == hydro.GAMER_EINVAL        # backward
-    assert L.gamer_hydro_advance_f64(None, None, 0, 3, 0.1, 1.0, 1.4, 1, None, None) == hydro.GAMER_OK
+    assert L.gamer_hydro_advance_f64_ex(a16, a16 + 8, 1, 3, 0.1, 1.0, 1.4, 0, None, None, None) == hydro.GAMER_EINVAL    # alignment
+    assert L.gamer_hydro_advance_f64_ex(a16, a16, 1, 3, 0.1, 0.0, 1.4, 0, None, None, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64_ex(a16, a16, 1, 3, 0.1, 1.0, 1.0, 0, None, None, None) == hydro.GAMER_EINVAL
+    assert L.gamer_hydro_advance_f64_ex(a16, a16, 1, 3, 0.1, 1.0, 1.4, 2, None, None, None) == hydro.GAMER_EINVAL        # backward
+    assert L.gamer_hydro_advance_f64_ex(None, None, 0, 3, 0.1, 1.0, 1.4, 1, None, None, None) == hydro.GAMER_OK
 
 
 def gpu_advance_f64(inp, dt, dh, gamma, backward=0):
@@ -37,8 +37,7 @@ def gpu_advance_f64(inp, dt, dh, gamma, backward=0):
     n = inp.shape[0]
     d_in = torch.from_numpy(np.ascontiguousarray(inp, np.float64)).cuda()
     d_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float64, device="cuda")
-    d_scr = torch.empty(hydro.gamer_hydro_f64_scratch_doubles(), dtype=torch.float64, device="cuda")
-    hydro.gamer_hydro_advance_f64(d_in, d_out, n, 3, dt, dh, gamma, d_scr, backward=backward)
+    hydro.gamer_hydro_advance_f64_ex(d_in, d_out, n, 3, dt, dh, gamma, backward=backward)
     torch.cuda.synchronize()
     return d_out.cpu().numpy()
 

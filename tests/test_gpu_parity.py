@@ -277,9 +277,10 @@ def test_runs_on_a_side_stream():
 def test_issue_probe_reports_plausible_clock_counts():
     """The measurement aid behind DESIGN.md 7: a 3-register FMA costs more than one issue slot and less than two; a
     warp-march (about 2 700 instructions) costs between 2 700 and 4 500 clocks and gets cheaper per slot with more warps."""
-    f3 = hydro.gamer_hydro_issue_probe(0, 4)
+    from paper_0907_3390_b200 import probes
+    f3 = probes.gamer_probe_issue(0, 4)
     assert 1.2 <= f3 <= 2.0, f3
     for what in (1, 2, 3):
-        c1, c4 = hydro.gamer_hydro_issue_probe(what, 1), hydro.gamer_hydro_issue_probe(what, 4)
+        c1, c4 = probes.gamer_probe_issue(what, 1), probes.gamer_probe_issue(what, 4)      # (fails if the state changed)
         assert 2700 <= c4 <= c1 <= 4500, (what, c1, c4)
 
