@@ -318,6 +318,20 @@ int gamer_hydro_pipeline_release(void) {
     return GAMER_OK;
 }
 
+// the ghost fill comes in two instantiations: the whole-strip walk, and the walk cut into segments for thin boxes
+static int prepare_ghost_fill(int* sm_count) {
+    int rc = prepare(reinterpret_cast<const void*>(gamer::ghost_fill_kernel<false>), 13, gamer::GF_SMEM_BYTES, sm_count);
+    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(gamer::ghost_fill_kernel<true>), 14, gamer::GF_SMEM_BYTES, sm_count);
+    return rc;
+}
+static void launch_ghost_fill(const float* d_interior, float* d_padded, const gamer::BoxGeom& geo, cudaStream_t stream) {
+    const unsigned int grid = (unsigned int)gamer::ghost_fill_ctas(geo.gx, geo.gy, geo.gz, geo.nseg);
+    if (geo.nseg > 1)
+        gamer::ghost_fill_kernel<true><<<grid, gamer::GF_THREADS, gamer::GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
+    else
+        gamer::ghost_fill_kernel<false><<<grid, gamer::GF_THREADS, gamer::GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
+}
+
 static int check_box(int gx, int gy, int gz, int bc_x, int bc_y, int bc_z) {
     if (gx < 1 || gy < 1 || gz < 1) return fail(GAMER_EINVAL, "box of %d x %d x %d groups", gx, gy, gz);
     if ((long long)gx * gy * gz * gamer::NCOMP > (1ll << 31) - 1) return fail(GAMER_EINVAL, "too many groups for one launch");
@@ -333,11 +347,10 @@ int gamer_hydro_ghost_fill(const float* d_interior, float* d_padded, int gx, int
     if (!aligned16(d_interior) || !aligned16(d_padded)) return fail(GAMER_EINVAL, "pointers must be 16-byte aligned");
     g_err[0] = '\0';
     int sm_count = 0;
-    rc = prepare(reinterpret_cast<const void*>(gamer::ghost_fill_kernel), 13, gamer::GF_SMEM_BYTES, &sm_count);
+    rc = prepare_ghost_fill(&sm_count);
     if (rc != GAMER_OK) return rc;
     gamer::BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}, gamer::ghost_fill_segments(gx, gy, gz, sm_count)};
-    gamer::ghost_fill_kernel<<<(unsigned int)gamer::ghost_fill_ctas(gx, gy, gz, geo.nseg), gamer::GF_THREADS, gamer::GF_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(
-        d_interior, d_padded, geo);
+    launch_ghost_fill(d_interior, d_padded, geo, static_cast<cudaStream_t>(stream));
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "ghost_fill launch: %s", cudaGetErrorString(e));
     return GAMER_OK;
@@ -372,13 +385,12 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
     int sm_count = 0;
     rc = prepare(reinterpret_cast<const void*>(fwd), order == 0 ? 8 : 11, SMEM_BYTES, &sm_count);
     if (rc == GAMER_OK && order == 1) rc = prepare(reinterpret_cast<const void*>(bwd), 12, SMEM_BYTES, &sm_count);
-    if (rc == GAMER_OK) rc = prepare(reinterpret_cast<const void*>(ghost_fill_kernel), 13, GF_SMEM_BYTES, &sm_count);
+    if (rc == GAMER_OK) rc = prepare_ghost_fill(&sm_count);
     if (rc != GAMER_OK) return rc;
     const int grid = (int)(n < (long long)sm_count ? n : (long long)sm_count);
     const int red_grid = (int)(n < 4ll * sm_count ? n : 4ll * sm_count);
     const unsigned int gsm_grid = (unsigned int)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024);
     BoxGeom geo{gx, gy, gz, {bc_x, bc_y, bc_z}, ghost_fill_segments(gx, gy, gz, sm_count)};
-    const unsigned int gf_grid = (unsigned int)ghost_fill_ctas(gx, gy, gz, geo.nseg);
     unsigned int* acc = reinterpret_cast<unsigned int*>(d_work);
     float* d_speed = d_work + 4;
     // Eq.30 over ALL padded cells (reading R10) costs one pass over the initial state.  After that the padded state
@@ -395,11 +407,11 @@ int gamer_hydro_run_uniform(float* d_padded, float* d_interior, int gx, int gy, 
         fwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr,
                                                          order == 0 ? d_speed : nullptr, d_work + 1);
         if (order == 1) {       // the backward sweep z,y,x follows with the SAME time step
-            ghost_fill_kernel<<<gf_grid, GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
+            launch_ghost_fill(d_interior, d_padded, geo, stream);
             bwd<<<grid, BLOCK_THREADS, SMEM_BYTES, stream>>>(d_padded, d_interior, n, gc, nullptr, d_speed, d_work + 1);
         }
         group_speed_max_kernel<<<gsm_grid, 256, 0, stream>>>(d_speed, n, acc);
-        ghost_fill_kernel<<<gf_grid, GF_THREADS, GF_SMEM_BYTES, stream>>>(d_interior, d_padded, geo);
+        launch_ghost_fill(d_interior, d_padded, geo, stream);
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) return fail(GAMER_ECUDA, "run_uniform: %s", cudaGetErrorString(e));

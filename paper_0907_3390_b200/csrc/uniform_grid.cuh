@@ -46,6 +46,8 @@ inline int ghost_fill_segments(int gx, int gy, int gz, int sm_count) {
 // number of CTAs that ghost_fill_kernel needs for a box of gx x gy x gz groups cut into nseg segments along x
 inline long long ghost_fill_ctas(int gx, int gy, int gz, int nseg = 1) { (void)gx; return (long long)gy * gz * NCOMP * nseg; }
 
+// SEGMENTED = false is the whole-strip walk (nseg == 1) with its bounds known at compile time: the code of round 2.
+template <bool SEGMENTED>
 __global__ void __launch_bounds__(GF_THREADS, 2)
 ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded, BoxGeom geo) {
     extern __shared__ __align__(128) unsigned char gf_smem[];
@@ -54,9 +56,11 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
     long long* const off_z = off_y + NP;
     const int v = blockIdx.x % NCOMP;
     const int strips = geo.gy * geo.gz;
-    const int strip = (blockIdx.x / NCOMP) % strips, seg = blockIdx.x / (NCOMP * strips);
+    const int strip = SEGMENTED ? (blockIdx.x / NCOMP) % strips : blockIdx.x / NCOMP;
+    const int seg = SEGMENTED ? blockIdx.x / (NCOMP * strips) : 0;
     const int ky = strip % geo.gy, kz = strip / geo.gy;
-    const int x0 = (int)((long long)seg * geo.gx / geo.nseg), x1 = (int)((long long)(seg + 1) * geo.gx / geo.nseg);
+    const int x0 = SEGMENTED ? (int)((long long)seg * geo.gx / geo.nseg) : 0;
+    const int x1 = SEGMENTED ? (int)((long long)(seg + 1) * geo.gx / geo.nseg) : geo.gx;
     // Per padded y and z: offset (in floats) of the source row inside `interior`, or -1 = beyond a "keep" end.
     constexpr long long GS = (long long)NCOMP * PS * PS * PS;     // floats per group of `interior`
     if (threadIdx.x < 2 * NP) {
