@@ -33,6 +33,7 @@ struct BoxGeom {
 //     one group early and ends one group late like the whole walk does, at the cost of one extra quarter-row load at
 //     each segment end.
 constexpr int GF_THREADS = 256;
+constexpr int GF_BAND = 8;                                        // z layers per band of strips (CTA numbering)
 constexpr int GF_ROWS = NP * NP;                                  // 484 padded (z,y) rows
 constexpr int GF_ITEMS = (GF_ROWS * 4 + GF_THREADS - 1) / GF_THREADS;   // 8 quarter rows per thread (the last one partial)
 constexpr int GF_SMEM_BYTES = 2 * VAR_FLOATS * 4 + 2 * NP * 8;    // two tiles + the y and z offset tables
@@ -58,7 +59,13 @@ ghost_fill_kernel(const float* __restrict__ interior, float* __restrict__ padded
     const int strips = geo.gy * geo.gz;
     const int strip = SEGMENTED ? (blockIdx.x / NCOMP) % strips : blockIdx.x / NCOMP;
     const int seg = SEGMENTED ? blockIdx.x / (NCOMP * strips) : 0;
-    const int ky = strip % geo.gy, kz = strip / geo.gy;
+    // Strips are numbered in bands of GF_BAND z layers, z fastest inside a band: the ~60 strips that are resident at
+    // the same time (2 CTAs per SM, 5 variables per strip) then form a block of about 7 x 8 in (ky, kz) that walks
+    // along x together, so that most y AND z neighbour rows a strip reads were just read by the strip that owns them
+    // and come from L2 instead of DRAM.  (All bands before the last are full, so band = strip / (GF_BAND * gy).)
+    const int band = strip / (GF_BAND * geo.gy), in_band = strip - band * (GF_BAND * geo.gy);
+    const int band_h = min(GF_BAND, geo.gz - band * GF_BAND);
+    const int ky = in_band / band_h, kz = band * GF_BAND + in_band % band_h;
     const int x0 = SEGMENTED ? (int)((long long)seg * geo.gx / geo.nseg) : 0;
     const int x1 = SEGMENTED ? (int)((long long)(seg + 1) * geo.gx / geo.nseg) : geo.gx;
     // Per padded y and z: offset (in floats) of the source row inside `interior`, or -1 = beyond a "keep" end.
